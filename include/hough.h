@@ -1,0 +1,178 @@
+/* hough.h -- C ABI of the B200-native conformal-mapped, matrix-form Hough
+ * transform (arxiv/paper_2607_04067; citations are PAPER.md line numbers).
+ *
+ * What the library computes, per event, entirely on the GPU (one fused kernel
+ * launch per hough_run call):
+ *   H0/H1  load the event's hits P = {(x_i, y_i)} and map them to
+ *          the conformal plane, u = x/(x^2+y^2), v = y/(x^2+y^2)  (Eq. (1));
+ *   H2     rho_ij = u_i cos(theta_j) + v_i sin(theta_j) for the shared theta
+ *          table, the matrix R of PAPER.md:92-96, binned at equal intervals
+ *          over [-rho_max, rho_max);
+ *   H3     vote every in-range (hit, theta_j) pair into the event's
+ *          N_theta x N_rho integer accumulator, held in shared memory
+ *          (block-local accumulation);
+ *   H4/H5  threshold + 3x3 local-maximum peaks, listed in raster order
+ *          (peak finding + NMS on the device);
+ *   H6     keep every hit whose own (theta, rho) bins fall inside any stored
+ *          peak's +-window (the hit filter of PAPER.md:44, :75);
+ *   H7     stable per-event compaction of the kept hits (N_select of Eq. (8),
+ *          PAPER.md:118-123).
+ * Arithmetic: fp32, round-to-nearest-even, one rounding per operation (no FMA
+ * contraction), IEEE division, denormals kept; integer results are exact.
+ * The exact operation order is DESIGN.md "Readings" S1-S6.
+ *
+ * Conventions
+ *   - Pointers named d_* are DEVICE pointers, h_* are HOST pointers.  The
+ *     caller owns every buffer it passes; the library owns only the handle,
+ *     its device copy of the cos/sin table and (for hough_run_host only) a
+ *     grow-only device staging area.
+ *   - hough_run / hough_run_ex are asynchronous on `stream`: they never
+ *     synchronise, never allocate, never read device data on the host, keep no
+ *     per-run scratch (one handle may be used from several streams at once)
+ *     and can be captured in a CUDA graph.
+ *   - All functions return 0 on success or a negative hough_status.
+ *   - There is no CPU fallback: without a CUDA device every call fails with
+ *     HOUGH_ERR_CUDA.
+ */
+#ifndef HOUGH_B200_H
+#define HOUGH_B200_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct hough_ctx hough_ctx;      /* opaque, library-owned */
+typedef void* hough_stream;              /* a cudaStream_t (CUstream); NULL = default stream */
+
+/* One peak (H5): accumulator cell (theta_bin, rho_bin) and its vote count. 8 bytes. */
+typedef struct hough_peak {
+    uint16_t theta_bin;
+    uint16_t rho_bin;
+    uint32_t votes;
+} hough_peak;
+
+typedef enum hough_status {
+    HOUGH_OK = 0,
+    HOUGH_ERR_INVALID_ARG = -1,   /* null pointer, out-of-range value */
+    HOUGH_ERR_UNSUPPORTED = -2,   /* grid does not fit even an 8-CTA cluster's shared memory */
+    HOUGH_ERR_CUDA = -3,          /* a CUDA call failed (no device, launch error, ...) */
+    HOUGH_ERR_NOMEM = -4          /* host or device allocation failed */
+} hough_status;
+
+typedef enum hough_option {
+    HOUGH_OPT_MAX_PEAKS = 1,        /* peaks stored per event, 0..1048576 (default 64) */
+    HOUGH_OPT_ACC_DTYPE = 2,        /* HOUGH_ACC_AUTO (= u16), HOUGH_ACC_U16, HOUGH_ACC_U32 */
+    HOUGH_OPT_CONFORMAL_SCALE = 3,  /* 1 (Eq. (1) as printed, default) or 2 (the scale Eq. (2) implies) */
+    HOUGH_OPT_CLUSTER_SIZE = 4,     /* 0 = smallest of {1,2,4,8} that fits (default), else force 1,2,4,8 */
+    HOUGH_OPT_CTAS_PER_SM = 5,      /* 0 = as many as fit, up to 2 (default); tuning knob */
+    HOUGH_OPT_VOTE_PATH = 6         /* 0 = fast packed-fp32 voting with the exact slow path only for
+                                       degenerate hits (default); 1 = force the slow path (testing) */
+} hough_option;
+
+enum { HOUGH_ACC_AUTO = 0, HOUGH_ACC_U16 = 1, HOUGH_ACC_U32 = 2 };
+
+typedef enum hough_info {
+    HOUGH_INFO_CLUSTER_SIZE = 1,    /* CTAs per event */
+    HOUGH_INFO_THREADS = 2,         /* threads per CTA */
+    HOUGH_INFO_SMEM_BYTES = 3,      /* dynamic shared memory per CTA */
+    HOUGH_INFO_CTAS_PER_SM = 4,     /* resident CTAs per SM (occupancy query) */
+    HOUGH_INFO_GRID_MAX = 5,        /* CTAs of a full persistent grid */
+    HOUGH_INFO_ACC_BITS = 6,        /* 16 or 32 */
+    HOUGH_INFO_MAX_PEAKS = 7,
+    HOUGH_INFO_CHUNK_HITS = 8,      /* hits staged in shared memory per pass */
+    HOUGH_INFO_SM_COUNT = 9,
+    HOUGH_INFO_LAUNCHES = 10        /* kernels launched through this handle so far */
+} hough_info;
+
+/* Creates a handle for an n_theta x n_rho accumulator over theta in [0, pi)
+ * (theta_j = j*pi/n_theta) and rho in [-rho_max, rho_max)
+ * (rho_max in 1/units of the hit coordinates), an absolute vote threshold
+ * (>= 1) and a keep window of +-window bins in theta and rho (>= 0).
+ * Builds the default cos/sin table ((float)cos((double)j*pi/n_theta)) and
+ * copies it to the device.  Requires 1 <= n_theta <= 65535, 1 <= n_rho <= 65535,
+ * rho_max finite and > 0.  Returns NULL on failure; hough_last_error() says why. */
+hough_ctx* hough_create(int n_theta, int n_rho, float rho_max, int threshold, int window);
+
+/* Sets an option (see hough_option).  Must not be called while a run that uses
+ * the handle is in flight.  HOUGH_ERR_UNSUPPORTED if the resulting
+ * configuration does not fit the device. */
+int hough_set_option(hough_ctx* ctx, int key, long long value);
+
+/* Replaces the theta table: h_cos[j], h_sin[j], j < n_theta, HOST pointers,
+ * copied (synchronously).  Values must be finite. */
+int hough_set_trig_table(hough_ctx* ctx, const float* h_cos, const float* h_sin);
+
+/* Reads a property of the current configuration (see hough_info); negative on error. */
+long long hough_get_info(const hough_ctx* ctx, int key);
+
+/* Runs H0-H7 on a batch (events are batched and independent).
+ *   d_xy            [n_total][2] fp32, interleaved (x, y); event e's hits are
+ *                   rows d_event_offsets[e] .. d_event_offsets[e+1]-1
+ *   d_event_offsets [n_events+1] int32, non-decreasing (CSR); not validated,
+ *                   decreasing offsets are undefined behaviour
+ *   d_keep_mask     [n_total] u8, written 0/1 for every hit
+ *   d_peaks         [n_events][max_peaks]; the first min(n_peaks, max_peaks)
+ *                   entries of an event are written, in raster order
+ *                   (theta_bin major, then rho_bin); the rest are untouched
+ *   d_counts        [n_events][2] int32 = {n_peaks found (untruncated), n_kept}
+ * An event with more than 65535 hits under a u16 accumulator gets counts
+ * {-1,-1} and no other output.  n_events == 0 is a successful no-op. */
+int hough_run(hough_ctx* ctx, const float* d_xy, const int32_t* d_event_offsets, int n_events,
+              uint8_t* d_keep_mask, hough_peak* d_peaks, int32_t* d_counts, hough_stream stream);
+
+/* hough_run plus optional outputs (any of the last three may be NULL):
+ *   d_kept_xy    [n_total][2] fp32 and
+ *   d_kept_idx   [n_total] int32: event e's kept hits, in original order, start
+ *                at d_event_offsets[e]; kept_idx is the index within the event;
+ *                entries past n_kept are untouched
+ *   d_accum_dump [n_events][n_theta][n_rho] u32: the accumulator (parity and
+ *                debugging only; never part of a timed run) */
+typedef struct hough_io {
+    const float* d_xy;
+    const int32_t* d_event_offsets;
+    int32_t n_events;
+    uint8_t* d_keep_mask;
+    hough_peak* d_peaks;
+    int32_t* d_counts;
+    float* d_kept_xy;
+    int32_t* d_kept_idx;
+    uint32_t* d_accum_dump;
+} hough_io;
+
+int hough_run_ex(hough_ctx* ctx, const hough_io* io, hough_stream stream);
+
+/* End-to-end form with HOST buffers (pinned memory recommended): copies
+ * h_xy / h_event_offsets to a library-owned device staging area, runs H0-H7
+ * and copies keep mask, peaks and counts (and kept_xy / kept_idx when not
+ * NULL) back, all asynchronously on `stream`; the host outputs are valid after
+ * the caller synchronises `stream`.  NOT re-entrant (the staging area belongs
+ * to the handle) and may allocate when a batch is larger than any before. */
+int hough_run_host(hough_ctx* ctx, const float* h_xy, const int32_t* h_event_offsets, int n_events,
+                   uint8_t* h_keep_mask, hough_peak* h_peaks, int32_t* h_counts,
+                   float* h_kept_xy, int32_t* h_kept_idx, hough_stream stream);
+
+/* Releases the handle and everything it owns.  NULL is allowed. */
+void hough_destroy(hough_ctx* ctx);
+
+const char* hough_strerror(int status);
+const char* hough_last_error(void);      /* thread-local message of the last failure */
+const char* hough_version(void);
+
+/* Measurement aid (the denominator of the vote roofline): times a
+ * kernel that does nothing but `iters` conflict-free no-return 32-bit shared
+ * atomic adds per thread, with `ctas_per_sm` x `threads` resident per SM, and
+ * returns atomics per second over the whole device in *out_rate.
+ *   variant 0: every lane its own bank, add of 1 (ATOMS.POPC.INC)
+ *   variant 1: every lane its own bank, add of a register value (ATOMS.ADD)
+ *   variant 2: pseudo-random bank per lane (natural bank conflicts)
+ *   variant 3: the voting loop's instruction mix without the atomics (issue bound)
+ *   variant 4: the voting loop's instruction mix with conflict-free atomics
+ * Synchronises the device. */
+int hough_bench_shared_atomics(int variant, int ctas_per_sm, int threads, long long iters, double* out_rate);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* HOUGH_B200_H */

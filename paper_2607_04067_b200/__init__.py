@@ -1,0 +1,265 @@
+"""paper_2607_04067_b200 -- thin Python binding of the C ABI in include/hough.h.
+
+Argument marshalling only: every step of the hot path (conformal map, rho
+matrix, voting, peaks, hit selection, compaction) runs in the CUDA kernels of
+libhough_b200.so.  PyTorch is used for device memory and streams.  There is no
+CPU fallback: if the library cannot be built/loaded or no CUDA device is
+present, calls raise.  This package never imports oracle/.
+"""
+import ctypes
+import os
+
+from . import build as _build
+
+HOUGH_OK = 0
+HOUGH_ERR_INVALID_ARG = -1
+HOUGH_ERR_UNSUPPORTED = -2
+HOUGH_ERR_CUDA = -3
+HOUGH_ERR_NOMEM = -4
+
+HOUGH_OPT_MAX_PEAKS = 1
+HOUGH_OPT_ACC_DTYPE = 2
+HOUGH_OPT_CONFORMAL_SCALE = 3
+HOUGH_OPT_CLUSTER_SIZE = 4
+HOUGH_OPT_CTAS_PER_SM = 5
+HOUGH_OPT_VOTE_PATH = 6
+HOUGH_ACC_AUTO, HOUGH_ACC_U16, HOUGH_ACC_U32 = 0, 1, 2
+
+HOUGH_INFO_CLUSTER_SIZE = 1
+HOUGH_INFO_THREADS = 2
+HOUGH_INFO_SMEM_BYTES = 3
+HOUGH_INFO_CTAS_PER_SM = 4
+HOUGH_INFO_GRID_MAX = 5
+HOUGH_INFO_ACC_BITS = 6
+HOUGH_INFO_MAX_PEAKS = 7
+HOUGH_INFO_CHUNK_HITS = 8
+HOUGH_INFO_SM_COUNT = 9
+HOUGH_INFO_LAUNCHES = 10
+
+EXPORTS = [
+    "hough_create", "hough_set_option", "hough_set_trig_table", "hough_get_info", "hough_run", "hough_run_ex",
+    "hough_run_host", "hough_destroy", "hough_strerror", "hough_last_error", "hough_version",
+    "hough_bench_shared_atomics",
+]
+
+
+class hough_io(ctypes.Structure):
+    _fields_ = [
+        ("d_xy", ctypes.c_void_p), ("d_event_offsets", ctypes.c_void_p), ("n_events", ctypes.c_int32),
+        ("d_keep_mask", ctypes.c_void_p), ("d_peaks", ctypes.c_void_p), ("d_counts", ctypes.c_void_p),
+        ("d_kept_xy", ctypes.c_void_p), ("d_kept_idx", ctypes.c_void_p), ("d_accum_dump", ctypes.c_void_p),
+    ]
+
+
+class HoughError(RuntimeError):
+    pass
+
+
+_lib = None
+
+
+def lib_path() -> str:
+    return _build.LIB
+
+
+def load_library():
+    """Loads (building first if the sources are newer) libhough_b200.so.  Raises if that fails."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    path = _build.build()
+    lib = ctypes.CDLL(path)
+    vp, ci, cll = ctypes.c_void_p, ctypes.c_int, ctypes.c_longlong
+    lib.hough_create.restype = vp
+    lib.hough_create.argtypes = [ci, ci, ctypes.c_float, ci, ci]
+    lib.hough_set_option.restype = ci
+    lib.hough_set_option.argtypes = [vp, ci, cll]
+    lib.hough_set_trig_table.restype = ci
+    lib.hough_set_trig_table.argtypes = [vp, vp, vp]
+    lib.hough_get_info.restype = cll
+    lib.hough_get_info.argtypes = [vp, ci]
+    lib.hough_run.restype = ci
+    lib.hough_run.argtypes = [vp, vp, vp, ci, vp, vp, vp, vp]
+    lib.hough_run_ex.restype = ci
+    lib.hough_run_ex.argtypes = [vp, ctypes.POINTER(hough_io), vp]
+    lib.hough_run_host.restype = ci
+    lib.hough_run_host.argtypes = [vp, vp, vp, ci, vp, vp, vp, vp, vp, vp]
+    lib.hough_destroy.restype = None
+    lib.hough_destroy.argtypes = [vp]
+    lib.hough_strerror.restype = ctypes.c_char_p
+    lib.hough_strerror.argtypes = [ci]
+    lib.hough_last_error.restype = ctypes.c_char_p
+    lib.hough_last_error.argtypes = []
+    lib.hough_version.restype = ctypes.c_char_p
+    lib.hough_version.argtypes = []
+    lib.hough_bench_shared_atomics.restype = ci
+    lib.hough_bench_shared_atomics.argtypes = [ci, ci, ci, cll, ctypes.POINTER(ctypes.c_double)]
+    _lib = lib
+    return lib
+
+
+def _check(rc, what):
+    if rc != HOUGH_OK:
+        lib = load_library()
+        raise HoughError("%s failed: %s (%s)" % (what, lib.hough_strerror(rc).decode(), lib.hough_last_error().decode()))
+
+
+_dummies = {}
+
+
+def _ptr(t):
+    """Address of a torch tensor (None -> NULL).  torch reports a null data_ptr() for a tensor with no
+    elements; the C ABI wants a real pointer for every required buffer, so an empty tensor is passed as
+    the address of a small per-device scratch allocation (never read or written: there are no elements)."""
+    if t is None:
+        return None
+    if t.numel() == 0:
+        import torch
+        key = (t.device.type, t.device.index)
+        if key not in _dummies:
+            _dummies[key] = torch.zeros(16, dtype=torch.uint8, device=t.device)
+        return ctypes.c_void_p(_dummies[key].data_ptr())
+    return ctypes.c_void_p(t.data_ptr())
+
+
+def _stream_handle(stream):
+    import torch
+    if stream is None:
+        stream = torch.cuda.current_stream()
+    return ctypes.c_void_p(stream.cuda_stream)
+
+
+# ---------------------------------------------------------------- same names as the C ABI
+def hough_create(n_theta, n_rho, rho_max, threshold, window):
+    lib = load_library()
+    ctx = lib.hough_create(n_theta, n_rho, ctypes.c_float(rho_max), threshold, window)
+    if not ctx:
+        raise HoughError("hough_create failed: " + lib.hough_last_error().decode())
+    return ctx
+
+
+def hough_set_option(ctx, key, value):
+    _check(load_library().hough_set_option(ctx, key, value), "hough_set_option")
+
+
+def hough_set_trig_table(ctx, h_cos, h_sin):
+    """h_cos, h_sin: contiguous float32 numpy arrays (HOST) of n_theta entries."""
+    import numpy as np
+    h_cos = np.ascontiguousarray(h_cos, dtype=np.float32)
+    h_sin = np.ascontiguousarray(h_sin, dtype=np.float32)
+    _check(load_library().hough_set_trig_table(ctx, h_cos.ctypes.data, h_sin.ctypes.data), "hough_set_trig_table")
+
+
+def hough_get_info(ctx, key):
+    return int(load_library().hough_get_info(ctx, key))
+
+
+def hough_run(ctx, d_xy, d_event_offsets, n_events, d_keep_mask, d_peaks, d_counts, stream=None):
+    """Tensors are CUDA torch tensors (see include/hough.h for shapes); asynchronous on `stream`."""
+    _check(load_library().hough_run(ctx, _ptr(d_xy), _ptr(d_event_offsets), n_events, _ptr(d_keep_mask),
+                                    _ptr(d_peaks), _ptr(d_counts), _stream_handle(stream)), "hough_run")
+
+
+def hough_run_ex(ctx, d_xy, d_event_offsets, n_events, d_keep_mask, d_peaks, d_counts,
+                 d_kept_xy=None, d_kept_idx=None, d_accum_dump=None, stream=None):
+    io = hough_io(_ptr(d_xy), _ptr(d_event_offsets), n_events, _ptr(d_keep_mask), _ptr(d_peaks), _ptr(d_counts),
+                  _ptr(d_kept_xy), _ptr(d_kept_idx), _ptr(d_accum_dump))
+    _check(load_library().hough_run_ex(ctx, ctypes.byref(io), _stream_handle(stream)), "hough_run_ex")
+
+
+def hough_run_host(ctx, h_xy, h_event_offsets, n_events, h_keep_mask, h_peaks, h_counts,
+                   h_kept_xy=None, h_kept_idx=None, stream=None):
+    """HOST (ideally pinned) torch tensors in and out; copies are inside the call, asynchronous on `stream`."""
+    _check(load_library().hough_run_host(ctx, _ptr(h_xy), _ptr(h_event_offsets), n_events, _ptr(h_keep_mask),
+                                         _ptr(h_peaks), _ptr(h_counts), _ptr(h_kept_xy), _ptr(h_kept_idx),
+                                         _stream_handle(stream)), "hough_run_host")
+
+
+def hough_destroy(ctx):
+    load_library().hough_destroy(ctx)
+
+
+def hough_version():
+    return load_library().hough_version().decode()
+
+
+def hough_bench_shared_atomics(variant, ctas_per_sm, threads, iters):
+    out = ctypes.c_double(0.0)
+    _check(load_library().hough_bench_shared_atomics(variant, ctas_per_sm, threads, iters, ctypes.byref(out)),
+           "hough_bench_shared_atomics")
+    return out.value
+
+
+# ---------------------------------------------------------------- convenience wrapper (allocation + marshalling only)
+class Hough:
+    """Owns a hough_ctx and allocates output tensors.  No arithmetic of the method happens here."""
+
+    def __init__(self, n_theta, n_rho, rho_max, threshold, window, max_peaks=64, acc_dtype="u16",
+                 conformal_scale=1, cluster_size=0, ctas_per_sm=0, trig_table=None):
+        self.n_theta, self.n_rho, self.max_peaks = n_theta, n_rho, max_peaks
+        self.ctx = hough_create(n_theta, n_rho, float(rho_max), threshold, window)
+        try:
+            hough_set_option(self.ctx, HOUGH_OPT_MAX_PEAKS, max_peaks)
+            hough_set_option(self.ctx, HOUGH_OPT_ACC_DTYPE, {"auto": 0, "u16": 1, "u32": 2}[acc_dtype])
+            if conformal_scale != 1:
+                hough_set_option(self.ctx, HOUGH_OPT_CONFORMAL_SCALE, conformal_scale)
+            if cluster_size:
+                hough_set_option(self.ctx, HOUGH_OPT_CLUSTER_SIZE, cluster_size)
+            if ctas_per_sm:
+                hough_set_option(self.ctx, HOUGH_OPT_CTAS_PER_SM, ctas_per_sm)
+            if trig_table is not None:
+                hough_set_trig_table(self.ctx, trig_table[0], trig_table[1])
+        except Exception:
+            self.close()
+            raise
+
+    def info(self, key):
+        return hough_get_info(self.ctx, key)
+
+    def alloc_outputs(self, n_total, n_events, device="cuda", kept=True, accum=False):
+        import torch
+        out = {
+            "keep": torch.zeros(max(n_total, 1), dtype=torch.uint8, device=device)[:n_total],
+            "peaks": torch.zeros((n_events, max(self.max_peaks, 1), 2), dtype=torch.int32, device=device)[:, :self.max_peaks],
+            "counts": torch.zeros((n_events, 2), dtype=torch.int32, device=device),
+        }
+        if kept:
+            out["kept_xy"] = torch.zeros((max(n_total, 1), 2), dtype=torch.float32, device=device)[:n_total]
+            out["kept_idx"] = torch.zeros(max(n_total, 1), dtype=torch.int32, device=device)[:n_total]
+        if accum:
+            out["accum"] = torch.zeros((n_events, self.n_theta, self.n_rho), dtype=torch.int32, device=device)
+        return out
+
+    def run(self, d_xy, d_offsets, out=None, stream=None, kept=True, accum=False):
+        """d_xy [N,2] f32 cuda, d_offsets [n_events+1] i32 cuda.  Returns the dict of output tensors
+        (peaks as int32 [n_events, max_peaks, 2]: word 0 = theta_bin | rho_bin << 16, word 1 = votes)."""
+        n_events = d_offsets.numel() - 1
+        n_total = d_xy.shape[0]
+        if out is None:
+            out = self.alloc_outputs(n_total, n_events, d_xy.device, kept=kept, accum=accum)
+        hough_run_ex(self.ctx, d_xy, d_offsets, n_events, out["keep"], out["peaks"], out["counts"],
+                     out.get("kept_xy"), out.get("kept_idx"), out.get("accum"), stream)
+        return out
+
+    def close(self):
+        if getattr(self, "ctx", None):
+            hough_destroy(self.ctx)
+            self.ctx = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+def unpack_peaks(peaks_i32):
+    """[n_events, max_peaks, 2] int32 (torch or numpy, on the host) -> numpy [n_events, max_peaks, 3] u32
+    (theta_bin, rho_bin, votes).  Pure bit unpacking of the hough_peak struct."""
+    import numpy as np
+    a = np.ascontiguousarray(peaks_i32.cpu().numpy() if hasattr(peaks_i32, "cpu") else peaks_i32).view(np.uint32)
+    out = np.empty(a.shape[:2] + (3,), dtype=np.uint32)
+    out[..., 0] = a[..., 0] & 0xFFFF
+    out[..., 1] = a[..., 0] >> 16
+    out[..., 2] = a[..., 1]
+    return out

@@ -1,0 +1,447 @@
+// hough_api.cu -- the C ABI of include/hough.h: handle management, shared-memory
+// planning, launch.  All compute is in hough_kernel.cuh; nothing here falls
+// back to the CPU.
+#include <atomic>
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "hough_kernel.cuh"
+
+using hough::KParams;
+
+namespace {
+
+thread_local char g_err[512] = "";
+
+int fail(int code, const char* fmt, ...) {
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof(g_err), fmt, ap);
+    va_end(ap);
+    return code;
+}
+
+#define CUDA_TRY(call)                                                                          \
+    do {                                                                                        \
+        cudaError_t _e = (call);                                                                \
+        if (_e != cudaSuccess) return fail(HOUGH_ERR_CUDA, "%s: %s", #call, cudaGetErrorString(_e)); \
+    } while (0)
+
+inline int align_up(int x, int a) { return (x + a - 1) / a * a; }
+
+struct Plan {
+    bool acc16 = true;
+    int csize = 1;
+    int threads = 0;
+    int smem_bytes = 0;
+    int ctas_per_sm = 0;     // measured with the occupancy API
+    int grid_max = 0;
+    KParams kp{};            // geometry part filled in; pointers per run
+};
+
+}  // namespace
+
+struct hough_ctx {
+    int n_theta, n_rho, threshold, window;
+    float rho_max, inv;
+    int max_peaks = 64;
+    int acc_dtype = HOUGH_ACC_AUTO;
+    int conformal_scale = 1;
+    int opt_cluster = 0;
+    int opt_ctas_per_sm = 0;
+    int opt_vote_path = 0;
+    int device = 0;
+    int sm_count = 0;
+    int smem_optin = 0;
+    float* d_cos = nullptr;
+    float* d_sin = nullptr;
+    float tmax = 1.0f;
+    Plan plan;
+    std::atomic<long long> launches{0};
+    // hough_run_host staging (grow-only)
+    long long cap_hits = 0;
+    int cap_events = 0;
+    long long cap_peaks = 0;
+    float* s_xy = nullptr;
+    int32_t* s_off = nullptr;
+    uint8_t* s_keep = nullptr;
+    hough_peak* s_peaks = nullptr;
+    int32_t* s_counts = nullptr;
+    float* s_kept_xy = nullptr;
+    int32_t* s_kept_idx = nullptr;
+};
+
+namespace {
+
+template <bool ACC16, bool CL>
+const void* kernel_ptr() { return (const void*)&hough::hough_event_kernel<ACC16, CL>; }
+
+const void* pick_kernel(bool acc16, bool cl) {
+    if (acc16) return cl ? kernel_ptr<true, true>() : kernel_ptr<true, false>();
+    return cl ? kernel_ptr<false, true>() : kernel_ptr<false, false>();
+}
+
+// Lays out shared memory for cluster size C and `want_ctas` CTAs per SM.  Returns false if it does not fit.
+bool try_plan(const hough_ctx* c, bool acc16, int C, int want_ctas, Plan* out) {
+    const int cols = (c->n_theta + C - 1) / C;
+    const int n_groups = (cols + 63) / 64;
+    const int max_warps = want_ctas >= 2 ? 16 : 32;
+    if (n_groups > max_warps) return false;
+    const int pitch_b = acc16 ? n_groups * 128 : n_groups * 256;
+    if (pitch_b > 8192) return false;
+    const long long acc_bytes = ((long long)c->n_rho + 1) * pitch_b;   // + the trash row
+    const int wpr = (c->n_rho + 31) / 32;
+    const int n_stripes = max_warps / n_groups;
+    const int threads = 32 * n_groups * n_stripes;
+    const int nwarps = threads / 32;
+    // post-extraction data that reuses the accumulator region
+    long long o = 0;
+    KParams kp{};
+    kp.d_off = (int)o;       o += align_up((c->n_theta + 1) * wpr * 4, 16);
+    kp.mcf_off = (int)o;     o += align_up((c->n_theta + 2) * 4, 16);
+    kp.msf_off = (int)o;     o += align_up((c->n_theta + 2) * 4, 16);
+    kp.mrow_off = (int)o;    o += align_up((c->n_theta + 2) * 4, 16);
+    kp.stash_off = (int)o;   o += (C > 1) ? align_up(HOUGH_SEL_ROUND_BLOCKS * nwarps * 4, 16) : 0;
+    kp.cnt_off = (int)o;     o += (C > 1) ? align_up(HOUGH_SEL_ROUND_BLOCKS * 4, 16) : 0;
+    kp.gcnt_off = (int)o;    o += (C > 1) ? align_up((HOUGH_SEL_ROUND_BLOCKS * C + 1) * 4, 16) : 0;
+    const long long region = align_up((int)std::max(acc_bytes, o), 16);
+    const long long pbm_bytes = align_up(cols * wpr * 4, 16);
+    const long long misc_bytes = 256;
+    const long long fixed = region + pbm_bytes + misc_bytes;
+    // per-CTA budget: the SM has 228 KB, each resident CTA reserves 1 KB; a single CTA may opt in to smem_optin
+    long long budget = (long long)(233472 / want_ctas) - 1024;
+    if (budget > c->smem_optin) budget = c->smem_optin;
+    long long chunk = (budget - fixed) / 8;
+    if (chunk < 128) return false;
+    if (chunk > 4096) chunk = 4096;
+    chunk &= ~1LL;
+    kp.csize = C;
+    kp.cols_per_cta = cols;
+    kp.n_groups = n_groups;
+    kp.n_stripes = n_stripes;
+    kp.pitch_b = pitch_b;
+    kp.wpr = wpr;
+    kp.chunk = (int)chunk;
+    kp.region_bytes = (int)region;
+    kp.pbm_off = (int)region;
+    kp.pbm_bytes = (int)pbm_bytes;
+    kp.hb_off = (int)(region + pbm_bytes);
+    kp.misc_off = kp.hb_off + (int)chunk * 8;
+    out->acc16 = acc16;
+    out->csize = C;
+    out->threads = threads;
+    out->smem_bytes = kp.misc_off + (int)misc_bytes;
+    out->kp = kp;
+    return true;
+}
+
+int make_plan(hough_ctx* c) {
+    const bool acc16 = c->acc_dtype != HOUGH_ACC_U32;
+    const int cands[4] = {1, 2, 4, 8};
+    Plan best;
+    bool found = false;
+    for (int ci = 0; ci < 4 && !found; ++ci) {
+        const int C = cands[ci];
+        if (c->opt_cluster && C != c->opt_cluster) continue;
+        if (C > c->n_theta) continue;
+        // prefer two CTAs per SM (phases of co-resident events overlap), else one
+        const int first = (c->opt_ctas_per_sm == 1) ? 1 : 2;
+        for (int want = first; want >= 1 && !found; --want) {
+            Plan pl;
+            if (try_plan(c, acc16, C, want, &pl)) { best = pl; found = true; }
+        }
+    }
+    if (!found)
+        return fail(HOUGH_ERR_UNSUPPORTED, "a %d x %d %s accumulator does not fit the shared memory of %s",
+                    c->n_theta, c->n_rho, acc16 ? "u16" : "u32",
+                    c->opt_cluster ? "the requested cluster size" : "an 8-CTA cluster");
+    const void* fn = pick_kernel(best.acc16, best.csize > 1);
+    CUDA_TRY(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, best.smem_bytes));
+    int occ = 0;
+    if (best.csize == 1) {
+        CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fn, best.threads, best.smem_bytes));
+        if (occ < 1) return fail(HOUGH_ERR_UNSUPPORTED, "kernel does not fit an SM (threads %d, smem %d)", best.threads, best.smem_bytes);
+        if (occ > 2) occ = 2;
+        best.ctas_per_sm = occ;
+        best.grid_max = occ * c->sm_count;
+    } else {
+        cudaLaunchConfig_t cfg{};
+        cfg.gridDim = dim3((unsigned)(c->sm_count / best.csize * best.csize));
+        cfg.blockDim = dim3((unsigned)best.threads);
+        cfg.dynamicSmemBytes = (size_t)best.smem_bytes;
+        cudaLaunchAttribute at{};
+        at.id = cudaLaunchAttributeClusterDimension;
+        at.val.clusterDim.x = (unsigned)best.csize; at.val.clusterDim.y = 1; at.val.clusterDim.z = 1;
+        cfg.attrs = &at; cfg.numAttrs = 1;
+        int ncl = 0;
+        CUDA_TRY(cudaOccupancyMaxActiveClusters(&ncl, fn, &cfg));
+        if (ncl < 1) return fail(HOUGH_ERR_UNSUPPORTED, "no %d-CTA cluster of this kernel fits the device", best.csize);
+        best.grid_max = ncl * best.csize;
+        best.ctas_per_sm = (best.grid_max + c->sm_count - 1) / c->sm_count;
+    }
+    c->plan = best;
+    return HOUGH_OK;
+}
+
+int upload_table(hough_ctx* c, const float* h_cos, const float* h_sin) {
+    float tmax = 0.0f;
+    for (int j = 0; j < c->n_theta; ++j) {
+        if (!std::isfinite(h_cos[j]) || !std::isfinite(h_sin[j]))
+            return fail(HOUGH_ERR_INVALID_ARG, "trig table entry %d is not finite", j);
+        tmax = std::fmax(tmax, std::fmax(std::fabs(h_cos[j]), std::fabs(h_sin[j])));
+    }
+    CUDA_TRY(cudaMemcpy(c->d_cos, h_cos, sizeof(float) * c->n_theta, cudaMemcpyHostToDevice));
+    CUDA_TRY(cudaMemcpy(c->d_sin, h_sin, sizeof(float) * c->n_theta, cudaMemcpyHostToDevice));
+    c->tmax = tmax;
+    return HOUGH_OK;
+}
+
+float tame_bound(const hough_ctx* c) {
+    // hits with (|u|+|v|) * tmax <= 0.99 * (2^17/inv - rho_max) have |t| < 2^17 at every column
+    double rho_lim = 131072.0 / (double)c->inv - (double)c->rho_max;
+    if (!(rho_lim > 0.0)) return 0.0f;
+    if (c->tmax <= 0.0f) return 3.0e38f;
+    double b = 0.99 * rho_lim / (double)c->tmax;
+    return b > 3.0e38 ? 3.0e38f : (float)b;
+}
+
+int launch(hough_ctx* c, const hough_io* io, cudaStream_t stream) {
+    const Plan& pl = c->plan;
+    KParams kp = pl.kp;
+    kp.xy = (const float2*)io->d_xy;
+    kp.off = io->d_event_offsets;
+    kp.n_events = io->n_events;
+    kp.keep = io->d_keep_mask;
+    kp.peaks = io->d_peaks;
+    kp.counts = io->d_counts;
+    kp.kept_xy = (float2*)io->d_kept_xy;
+    kp.kept_idx = io->d_kept_idx;
+    kp.accum_dump = io->d_accum_dump;
+    kp.cos_t = c->d_cos;
+    kp.sin_t = c->d_sin;
+    kp.n_theta = c->n_theta; kp.n_rho = c->n_rho; kp.threshold = c->threshold; kp.window = c->window;
+    kp.max_peaks = c->max_peaks;
+    kp.rho_max = c->rho_max; kp.inv = c->inv; kp.scale = (float)c->conformal_scale;
+    kp.tame_bound = tame_bound(c);
+    kp.force_slow = c->opt_vote_path == 1;
+    const int C = pl.csize;
+    long long want = (long long)io->n_events * C;
+    int grid = (int)std::min<long long>(want, pl.grid_max);
+    grid = grid / C * C;
+    if (grid < C) grid = C;
+    const void* fn = pick_kernel(pl.acc16, C > 1);
+    cudaLaunchConfig_t cfg{};
+    cfg.gridDim = dim3((unsigned)grid);
+    cfg.blockDim = dim3((unsigned)pl.threads);
+    cfg.dynamicSmemBytes = (size_t)pl.smem_bytes;
+    cfg.stream = stream;
+    cudaLaunchAttribute at{};
+    if (C > 1) {
+        at.id = cudaLaunchAttributeClusterDimension;
+        at.val.clusterDim.x = (unsigned)C; at.val.clusterDim.y = 1; at.val.clusterDim.z = 1;
+        cfg.attrs = &at; cfg.numAttrs = 1;
+    }
+    void* args[1] = {(void*)&kp};
+    CUDA_TRY(cudaLaunchKernelExC(&cfg, fn, args));
+    c->launches.fetch_add(1);
+    return HOUGH_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+hough_ctx* hough_create(int n_theta, int n_rho, float rho_max, int threshold, int window) {
+    if (n_theta < 1 || n_theta > 65535 || n_rho < 1 || n_rho > 65535) {
+        fail(HOUGH_ERR_INVALID_ARG, "n_theta and n_rho must be in 1..65535 (got %d, %d)", n_theta, n_rho);
+        return nullptr;
+    }
+    if (!(rho_max > 0.0f) || !std::isfinite(rho_max)) { fail(HOUGH_ERR_INVALID_ARG, "rho_max must be finite and > 0"); return nullptr; }
+    if (threshold < 1) { fail(HOUGH_ERR_INVALID_ARG, "threshold must be >= 1"); return nullptr; }
+    if (window < 0 || window > 65535) { fail(HOUGH_ERR_INVALID_ARG, "window must be in 0..65535"); return nullptr; }
+    int ndev = 0;
+    cudaError_t e = cudaGetDeviceCount(&ndev);
+    if (e != cudaSuccess || ndev < 1) {
+        fail(HOUGH_ERR_CUDA, "no CUDA device (%s); this library has no CPU fallback", cudaGetErrorString(e));
+        return nullptr;
+    }
+    hough_ctx* c = new (std::nothrow) hough_ctx();
+    if (!c) { fail(HOUGH_ERR_NOMEM, "out of host memory"); return nullptr; }
+    c->n_theta = n_theta; c->n_rho = n_rho; c->rho_max = rho_max; c->threshold = threshold; c->window = window;
+    c->inv = (float)((double)n_rho / (2.0 * (double)rho_max));
+    cudaDeviceProp prop;
+    if (cudaGetDevice(&c->device) != cudaSuccess || cudaGetDeviceProperties(&prop, c->device) != cudaSuccess) {
+        fail(HOUGH_ERR_CUDA, "cannot query the current CUDA device");
+        delete c; return nullptr;
+    }
+    if (prop.major < 10) {
+        fail(HOUGH_ERR_UNSUPPORTED, "built for sm_100a (B200); device is sm_%d%d", prop.major, prop.minor);
+        delete c; return nullptr;
+    }
+    c->sm_count = prop.multiProcessorCount;
+    c->smem_optin = (int)prop.sharedMemPerBlockOptin;
+    if (cudaMalloc(&c->d_cos, sizeof(float) * n_theta) != cudaSuccess || cudaMalloc(&c->d_sin, sizeof(float) * n_theta) != cudaSuccess) {
+        fail(HOUGH_ERR_NOMEM, "cudaMalloc of the trig table failed");
+        hough_destroy(c); return nullptr;
+    }
+    std::vector<float> hc(n_theta), hs(n_theta);
+    for (int j = 0; j < n_theta; ++j) {   // theta_j = j*pi/n_theta, left bin edges (reading Q3)
+        double th = (double)j * M_PI / (double)n_theta;
+        hc[j] = (float)std::cos(th);
+        hs[j] = (float)std::sin(th);
+    }
+    if (upload_table(c, hc.data(), hs.data()) != HOUGH_OK || make_plan(c) != HOUGH_OK) { hough_destroy(c); return nullptr; }
+    return c;
+}
+
+int hough_set_option(hough_ctx* c, int key, long long value) {
+    if (!c) return fail(HOUGH_ERR_INVALID_ARG, "null handle");
+    const int o_mp = c->max_peaks, o_acc = c->acc_dtype, o_sc = c->conformal_scale, o_cl = c->opt_cluster,
+              o_cps = c->opt_ctas_per_sm, o_vp = c->opt_vote_path;
+    switch (key) {
+        case HOUGH_OPT_MAX_PEAKS:
+            if (value < 0 || value > 1048576) return fail(HOUGH_ERR_INVALID_ARG, "max_peaks must be in 0..1048576");
+            c->max_peaks = (int)value; return HOUGH_OK;
+        case HOUGH_OPT_ACC_DTYPE:
+            if (value != HOUGH_ACC_AUTO && value != HOUGH_ACC_U16 && value != HOUGH_ACC_U32) return fail(HOUGH_ERR_INVALID_ARG, "bad accumulator dtype");
+            c->acc_dtype = (int)value; break;
+        case HOUGH_OPT_CONFORMAL_SCALE:
+            if (value != 1 && value != 2) return fail(HOUGH_ERR_INVALID_ARG, "conformal scale must be 1 or 2");
+            c->conformal_scale = (int)value; return HOUGH_OK;
+        case HOUGH_OPT_CLUSTER_SIZE:
+            if (value != 0 && value != 1 && value != 2 && value != 4 && value != 8) return fail(HOUGH_ERR_INVALID_ARG, "cluster size must be 0,1,2,4,8");
+            c->opt_cluster = (int)value; break;
+        case HOUGH_OPT_CTAS_PER_SM:
+            if (value < 0 || value > 2) return fail(HOUGH_ERR_INVALID_ARG, "ctas_per_sm must be 0,1,2");
+            c->opt_ctas_per_sm = (int)value; break;
+        case HOUGH_OPT_VOTE_PATH:
+            if (value != 0 && value != 1) return fail(HOUGH_ERR_INVALID_ARG, "vote path must be 0 or 1");
+            c->opt_vote_path = (int)value; return HOUGH_OK;
+        default:
+            return fail(HOUGH_ERR_INVALID_ARG, "unknown option %d", key);
+    }
+    int rc = make_plan(c);
+    if (rc != HOUGH_OK) {   // roll back: the handle stays usable with its previous configuration
+        c->max_peaks = o_mp; c->acc_dtype = o_acc; c->conformal_scale = o_sc; c->opt_cluster = o_cl;
+        c->opt_ctas_per_sm = o_cps; c->opt_vote_path = o_vp;
+    }
+    return rc;
+}
+
+int hough_set_trig_table(hough_ctx* c, const float* h_cos, const float* h_sin) {
+    if (!c || !h_cos || !h_sin) return fail(HOUGH_ERR_INVALID_ARG, "null argument");
+    return upload_table(c, h_cos, h_sin);
+}
+
+long long hough_get_info(const hough_ctx* c, int key) {
+    if (!c) return fail(HOUGH_ERR_INVALID_ARG, "null handle");
+    switch (key) {
+        case HOUGH_INFO_CLUSTER_SIZE: return c->plan.csize;
+        case HOUGH_INFO_THREADS: return c->plan.threads;
+        case HOUGH_INFO_SMEM_BYTES: return c->plan.smem_bytes;
+        case HOUGH_INFO_CTAS_PER_SM: return c->plan.ctas_per_sm;
+        case HOUGH_INFO_GRID_MAX: return c->plan.grid_max;
+        case HOUGH_INFO_ACC_BITS: return c->plan.acc16 ? 16 : 32;
+        case HOUGH_INFO_MAX_PEAKS: return c->max_peaks;
+        case HOUGH_INFO_CHUNK_HITS: return c->plan.kp.chunk;
+        case HOUGH_INFO_SM_COUNT: return c->sm_count;
+        case HOUGH_INFO_LAUNCHES: return c->launches.load();
+        default: return fail(HOUGH_ERR_INVALID_ARG, "unknown info key %d", key);
+    }
+}
+
+int hough_run_ex(hough_ctx* c, const hough_io* io, hough_stream stream) {
+    if (!c || !io) return fail(HOUGH_ERR_INVALID_ARG, "null handle or io");
+    if (io->n_events < 0) return fail(HOUGH_ERR_INVALID_ARG, "n_events < 0");
+    if (io->n_events == 0) return HOUGH_OK;
+    if (!io->d_xy || !io->d_event_offsets || !io->d_keep_mask || !io->d_counts) return fail(HOUGH_ERR_INVALID_ARG, "null device pointer");
+    if (!io->d_peaks && c->max_peaks > 0) return fail(HOUGH_ERR_INVALID_ARG, "d_peaks is null but max_peaks > 0");
+    return launch(c, io, (cudaStream_t)stream);
+}
+
+int hough_run(hough_ctx* c, const float* d_xy, const int32_t* d_event_offsets, int n_events,
+              uint8_t* d_keep_mask, hough_peak* d_peaks, int32_t* d_counts, hough_stream stream) {
+    hough_io io{};
+    io.d_xy = d_xy; io.d_event_offsets = d_event_offsets; io.n_events = n_events;
+    io.d_keep_mask = d_keep_mask; io.d_peaks = d_peaks; io.d_counts = d_counts;
+    return hough_run_ex(c, &io, stream);
+}
+
+int hough_run_host(hough_ctx* c, const float* h_xy, const int32_t* h_off, int n_events,
+                   uint8_t* h_keep, hough_peak* h_peaks, int32_t* h_counts,
+                   float* h_kept_xy, int32_t* h_kept_idx, hough_stream stream) {
+    if (!c) return fail(HOUGH_ERR_INVALID_ARG, "null handle");
+    if (n_events < 0) return fail(HOUGH_ERR_INVALID_ARG, "n_events < 0");
+    if (n_events == 0) return HOUGH_OK;
+    if (!h_off || !h_keep || !h_counts || (!h_peaks && c->max_peaks > 0)) return fail(HOUGH_ERR_INVALID_ARG, "null host pointer");
+    const long long n_total = (long long)h_off[n_events] ;
+    if (n_total < 0 || (n_total > 0 && !h_xy)) return fail(HOUGH_ERR_INVALID_ARG, "bad offsets or null h_xy");
+    cudaStream_t st = (cudaStream_t)stream;
+    const long long n_peaks_cap = (long long)n_events * c->max_peaks;
+    if (n_total > c->cap_hits || n_events > c->cap_events || n_peaks_cap > c->cap_peaks) {
+        CUDA_TRY(cudaStreamSynchronize(st));
+        cudaFree(c->s_xy); cudaFree(c->s_off); cudaFree(c->s_keep); cudaFree(c->s_peaks); cudaFree(c->s_counts);
+        cudaFree(c->s_kept_xy); cudaFree(c->s_kept_idx);
+        c->s_xy = nullptr; c->s_off = nullptr; c->s_keep = nullptr; c->s_peaks = nullptr; c->s_counts = nullptr;
+        c->s_kept_xy = nullptr; c->s_kept_idx = nullptr;
+        c->cap_hits = std::max<long long>(n_total, c->cap_hits) + 16;
+        c->cap_events = std::max(n_events, c->cap_events);
+        c->cap_peaks = std::max<long long>(n_peaks_cap, c->cap_peaks) + 1;
+        cudaError_t e1 = cudaMalloc(&c->s_xy, sizeof(float) * 2 * c->cap_hits);
+        cudaError_t e2 = cudaMalloc(&c->s_off, sizeof(int32_t) * ((size_t)c->cap_events + 1));
+        cudaError_t e3 = cudaMalloc(&c->s_keep, (size_t)c->cap_hits);
+        cudaError_t e4 = cudaMalloc(&c->s_peaks, sizeof(hough_peak) * (size_t)c->cap_peaks);
+        cudaError_t e5 = cudaMalloc(&c->s_counts, sizeof(int32_t) * 2 * (size_t)c->cap_events);
+        cudaError_t e6 = cudaMalloc(&c->s_kept_xy, sizeof(float) * 2 * c->cap_hits);
+        cudaError_t e7 = cudaMalloc(&c->s_kept_idx, sizeof(int32_t) * c->cap_hits);
+        if (e1 || e2 || e3 || e4 || e5 || e6 || e7) {
+            c->cap_hits = 0; c->cap_events = 0; c->cap_peaks = 0;
+            return fail(HOUGH_ERR_NOMEM, "cudaMalloc of the staging area failed");
+        }
+    }
+    if (n_total > 0) CUDA_TRY(cudaMemcpyAsync(c->s_xy, h_xy, sizeof(float) * 2 * n_total, cudaMemcpyHostToDevice, st));
+    CUDA_TRY(cudaMemcpyAsync(c->s_off, h_off, sizeof(int32_t) * ((size_t)n_events + 1), cudaMemcpyHostToDevice, st));
+    hough_io io{};
+    io.d_xy = c->s_xy; io.d_event_offsets = c->s_off; io.n_events = n_events;
+    io.d_keep_mask = c->s_keep; io.d_peaks = c->s_peaks; io.d_counts = c->s_counts;
+    io.d_kept_xy = h_kept_xy ? c->s_kept_xy : nullptr;
+    io.d_kept_idx = h_kept_idx ? c->s_kept_idx : nullptr;
+    int rc = launch(c, &io, st);
+    if (rc != HOUGH_OK) return rc;
+    if (n_total > 0) CUDA_TRY(cudaMemcpyAsync(h_keep, c->s_keep, (size_t)n_total, cudaMemcpyDeviceToHost, st));
+    if (c->max_peaks > 0) CUDA_TRY(cudaMemcpyAsync(h_peaks, c->s_peaks, sizeof(hough_peak) * (size_t)n_peaks_cap, cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(cudaMemcpyAsync(h_counts, c->s_counts, sizeof(int32_t) * 2 * (size_t)n_events, cudaMemcpyDeviceToHost, st));
+    if (h_kept_xy && n_total > 0) CUDA_TRY(cudaMemcpyAsync(h_kept_xy, c->s_kept_xy, sizeof(float) * 2 * n_total, cudaMemcpyDeviceToHost, st));
+    if (h_kept_idx && n_total > 0) CUDA_TRY(cudaMemcpyAsync(h_kept_idx, c->s_kept_idx, sizeof(int32_t) * n_total, cudaMemcpyDeviceToHost, st));
+    return HOUGH_OK;
+}
+
+void hough_destroy(hough_ctx* c) {
+    if (!c) return;
+    cudaFree(c->d_cos); cudaFree(c->d_sin);
+    cudaFree(c->s_xy); cudaFree(c->s_off); cudaFree(c->s_keep); cudaFree(c->s_peaks); cudaFree(c->s_counts);
+    cudaFree(c->s_kept_xy); cudaFree(c->s_kept_idx);
+    delete c;
+}
+
+const char* hough_strerror(int status) {
+    switch (status) {
+        case HOUGH_OK: return "ok";
+        case HOUGH_ERR_INVALID_ARG: return "invalid argument";
+        case HOUGH_ERR_UNSUPPORTED: return "unsupported configuration";
+        case HOUGH_ERR_CUDA: return "CUDA error";
+        case HOUGH_ERR_NOMEM: return "out of memory";
+        default: return "unknown status";
+    }
+}
+
+const char* hough_last_error(void) { return g_err; }
+
+const char* hough_version(void) { return "hough-b200 0.1 (sm_100a)"; }
+
+}  // extern "C"

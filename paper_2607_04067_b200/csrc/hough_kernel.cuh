@@ -1,0 +1,511 @@
+// hough_kernel.cuh -- the fused per-event kernel (sm_100a).
+//
+// One CTA (or one thread-block cluster of C CTAs that split the theta columns)
+// owns one event at a time and walks a static round-robin list of events
+// (persistent grid, no scratch, re-entrant across streams).  Per event:
+//   H0/H1 stage hits -> conformal (u,v) in shared memory   PAPER.md:52-57 Eq. (1)
+//   H2/H3 vote: lane = theta column, warp-uniform hit
+//   H4    threshold + 3x3 local maximum -> peak bitmap
+//   H5    raster-order peak list
+//   H6    hit selection against the dilated peak bitmap
+//   H7    stable compaction
+// The exact fp32 operation order is DESIGN.md S1/S2 (one rounding per
+// operation, no FMA contraction).  This file shares nothing with oracle/.
+//
+// Accumulator layout in shared memory: rho-major,
+// A[k][word], so that a warp that owns 32 (or 64) adjacent theta columns hits
+// 32 distinct banks whatever the rho bins are: votes are conflict-free by
+// construction.  Local column jl = 64 g + 32 h + l  (group g, half h, lane l):
+//   u16: word g*32 + l of row k holds columns (h=0 | h=1) in its (low | high) half
+//   u32: word (2g+h)*32 + l of row k
+// Row n_rho is a trash row that swallows the out-of-range votes (never scanned).
+#pragma once
+#include <cooperative_groups.h>
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/hough.h"
+
+namespace hough {
+namespace cg = cooperative_groups;
+
+typedef unsigned long long ull;
+
+// 1.5 * 2^23: adding it with round-toward-minus-infinity leaves floor(t) in the
+// low mantissa bits for |t| < 2^22 (exact: the sum is representable up to the
+// rounding that IS the floor).
+#define HOUGH_MAGIC_F 12582912.0f
+#define HOUGH_MAGIC_BITS 0x4B400000u
+#define HOUGH_SEL_ROUND_BLOCKS 32   // clustered selection: hit blocks per CTA per round
+
+struct KParams {
+    const float2* xy;
+    const int* off;
+    int n_events;
+    unsigned char* keep;
+    hough_peak* peaks;
+    int* counts;
+    float2* kept_xy;
+    int* kept_idx;
+    unsigned* accum_dump;
+    const float* cos_t;
+    const float* sin_t;
+    int n_theta, n_rho, threshold, window, max_peaks;
+    float rho_max, inv, scale;
+    float tame_bound;     // a hit is "tame" iff (|u|+|v|) <= tame_bound (then |t| < 2^17 at every column)
+    int force_slow;
+    int csize;            // CTAs per event (cluster size)
+    int cols_per_cta;     // theta columns owned by one CTA
+    int n_groups;         // 64-column groups per CTA
+    int n_stripes;        // warps per group in the vote phase
+    int pitch_b;          // bytes per rho row of the accumulator (multiple of 128)
+    int wpr;              // 32-bit words per bitmap row = ceil(n_rho / 32)
+    int chunk;            // hits staged per pass
+    int region_bytes;     // accumulator region (also reused after peak extraction)
+    int pbm_off;          // peak bitmap [cols_per_cta][wpr]
+    int pbm_bytes;
+    int hb_off;           // hit buffer float2[chunk]
+    int misc_off;         // 64 ints
+    // post-extraction layout inside the accumulator region (byte offsets)
+    int d_off, mcf_off, msf_off, mrow_off, stash_off, cnt_off, gcnt_off;
+};
+
+// ---------------------------------------------------------------- small helpers
+__device__ __forceinline__ void red_shared_add(unsigned saddr, unsigned v) {
+    asm volatile("red.shared.add.u32 [%0], %1;" ::"r"(saddr), "r"(v) : "memory");
+}
+// The vote proper.  No "memory" clobber: ordering against the zeroing stores and the later scan is
+// given by the __syncthreads() around the vote phase, and the compiler stays free to hoist the
+// hit loads of the next iterations above it.
+__device__ __forceinline__ void vote_add(unsigned saddr, unsigned v) {
+    asm volatile("red.shared.add.u32 [%0], %1;" ::"r"(saddr), "r"(v));
+}
+__device__ __forceinline__ void red_shared_or(unsigned saddr, unsigned v) {
+    asm volatile("red.shared.or.b32 [%0], %1;" ::"r"(saddr), "r"(v) : "memory");
+}
+
+// S1: d = fl(fl(x*x)+fl(y*y)); u = scale*fl(x/d); v = scale*fl(y/d).  Eq. (1).
+__device__ __forceinline__ float2 conformal(float2 h, float scale) {
+    float d = __fadd_rn(__fmul_rn(h.x, h.x), __fmul_rn(h.y, h.y));
+    return make_float2(__fmul_rn(scale, __fdiv_rn(h.x, d)), __fmul_rn(scale, __fdiv_rn(h.y, d)));
+}
+
+// S2 for one (hit, theta column) pair, one rounding per operation, intrinsics that ptxas never contracts:
+//   rho = fl(fl(u*c) + fl(v*s)); t = fl(fl(rho + rho_max) * inv); y = t + 1.5*2^23 rounded toward -inf.
+// Returns the raw bits of y: (bits - HOUGH_MAGIC_BITS) as unsigned is < n_rho  <=>  0 <= t < n_rho, and
+// then it IS floor(t) -- for every input, including NaN/inf/huge.
+// (Packed fp32x2 instructions were measured on B200 to take two issue slots each, so they buy nothing
+// in this issue-bound loop and they invite FFMA2 contraction; profiles/r01_microbench.md.)
+__device__ __forceinline__ unsigned bin_bits(float u, float v, float c, float s, float rho_max, float inv) {
+    const float rho = __fadd_rn(__fmul_rn(u, c), __fmul_rn(v, s));
+    const float t = __fmul_rn(__fadd_rn(rho, rho_max), inv);
+    return __float_as_uint(__fadd_rd(t, HOUGH_MAGIC_F));
+}
+
+// S2, scalar and literal (the slow exact path and the reference for the trick).  Returns k or -1.
+__device__ __forceinline__ int bin_exact(float u, float v, float c, float s, float rho_max, float inv, int n_rho) {
+    float rho = __fadd_rn(__fmul_rn(u, c), __fmul_rn(v, s));
+    float t = __fmul_rn(__fadd_rn(rho, rho_max), inv);
+    if (t >= 0.0f && t < (float)n_rho) return (int)t;
+    return -1;
+}
+
+// Exclusive scan of one int per thread over the CTA; `total` is returned to every thread.
+// wsum: 33 ints of shared scratch.  Contains two __syncthreads().
+__device__ __forceinline__ int block_exscan(int v, int* wsum, int& total) {
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarps = (blockDim.x + 31) >> 5;
+    int inc = v;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+        int o = __shfl_up_sync(0xffffffffu, inc, d);
+        if (lane >= d) inc += o;
+    }
+    if (lane == 31) wsum[warp] = inc;
+    __syncthreads();
+    if (warp == 0) {
+        int w = lane < nwarps ? wsum[lane] : 0;
+        int winc = w;
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) {
+            int o = __shfl_up_sync(0xffffffffu, winc, d);
+            if (lane >= d) winc += o;
+        }
+        wsum[lane] = winc - w;
+        if (lane == 31) wsum[32] = winc;
+    }
+    __syncthreads();
+    total = wsum[32];
+    int r = wsum[warp] + inc - v;
+    return r;
+}
+
+template <bool ACC16>
+__device__ __forceinline__ unsigned cell_word_off(int jl) {   // word index within a rho row
+    int g = jl >> 6, h = (jl >> 5) & 1, l = jl & 31;
+    return ACC16 ? (unsigned)(g * 32 + l) : (unsigned)((2 * g + h) * 32 + l);
+}
+
+template <bool ACC16>
+__device__ __forceinline__ unsigned cell_from(const unsigned char* acc, int pitch_b, int jl, int k) {
+    unsigned w = *(const unsigned*)(acc + (size_t)k * pitch_b + 4u * cell_word_off<ACC16>(jl));
+    if (ACC16) return (w >> (16 * ((jl >> 5) & 1))) & 0xFFFFu;
+    return w;
+}
+
+// ---------------------------------------------------------------- the kernel
+template <bool ACC16, bool CL>
+__global__ void __launch_bounds__(1024, 1) hough_event_kernel(const __grid_constant__ KParams p) {
+    extern __shared__ __align__(128) unsigned char smem[];
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int nthreads = blockDim.x, nwarps = nthreads >> 5;
+
+    unsigned rank = 0;
+    if (CL) rank = cg::this_cluster().block_rank();
+    const int C = p.csize;
+    const int cluster_id = blockIdx.x / C, n_clusters = gridDim.x / C;
+
+    unsigned char* acc = smem;                                  // accumulator region
+    unsigned* pbm = (unsigned*)(smem + p.pbm_off);              // peak bitmap [cols_per_cta][wpr]
+    float2* hb = (float2*)(smem + p.hb_off);                    // staged (u,v)
+    int* misc = (int*)(smem + p.misc_off);                      // [0..32] scan scratch, [40] peak total, [41] marked count
+    const unsigned acc_s = (unsigned)__cvta_generic_to_shared(acc);
+
+    const int col0 = (int)rank * p.cols_per_cta;
+    int ncols = p.n_theta - col0;
+    if (ncols > p.cols_per_cta) ncols = p.cols_per_cta;
+    if (ncols < 0) ncols = 0;
+
+    // ---- vote-phase lane constants: this lane owns local columns jl0 and jl0+32 of group g
+    const int g = warp % p.n_groups, stripe = warp / p.n_groups;
+    const int jl0 = 64 * g + lane, jl1 = jl0 + 32;
+    const bool valid0 = jl0 < ncols, valid1 = jl1 < ncols;
+    const float c0 = valid0 ? p.cos_t[col0 + jl0] : 0.0f, s0 = valid0 ? p.sin_t[col0 + jl0] : 0.0f;
+    const float c1 = valid1 ? p.cos_t[col0 + jl1] : 0.0f, s1 = valid1 ? p.sin_t[col0 + jl1] : 0.0f;
+    const unsigned woff0 = 4u * cell_word_off<ACC16>(jl0), woff1 = 4u * cell_word_off<ACC16>(jl1);
+    const unsigned inc0 = 1u, inc1 = ACC16 ? 0x10000u : 1u;
+    const unsigned pitch = (unsigned)p.pitch_b;
+    const unsigned limit = (unsigned)p.n_rho * pitch;
+    // rel = (bits - MAGIC_BITS) * pitch + woff ; invalid columns are pushed out of range for good
+    const unsigned lc0 = (valid0 ? woff0 : 0x80000000u) - HOUGH_MAGIC_BITS * pitch;
+    const unsigned lc1 = (valid1 ? woff1 : 0x80000000u) - HOUGH_MAGIC_BITS * pitch;
+    const unsigned trash0 = limit + woff0, trash1 = limit + woff1;
+    const float rho_max = p.rho_max, inv = p.inv;
+
+    const int zero_vec = (p.region_bytes + p.pbm_bytes) >> 4;   // pbm follows the region; both 16-B multiples
+
+    for (int e = cluster_id; e < p.n_events; e += n_clusters) {
+        // shfl from lane 0 = "this value is warp-uniform" for ptxas (keeps the event loop in uniform control flow)
+        const int beg = __shfl_sync(0xffffffffu, p.off[e], 0);
+        const int n = __shfl_sync(0xffffffffu, p.off[e + 1], 0) - beg;
+        if (ACC16 && n > 65535) {   // a u16 cell could wrap: refuse the event (uniform over the cluster)
+            if (rank == 0 && tid == 0) { p.counts[2 * e] = -1; p.counts[2 * e + 1] = -1; }
+            continue;
+        }
+
+        // ---- zero accumulator + peak bitmap
+        {
+            uint4* z = (uint4*)smem;
+            const uint4 zz = make_uint4(0, 0, 0, 0);
+            for (int i = tid; i < zero_vec; i += nthreads) z[i] = zz;
+        }
+
+        // ---- H0-H3: stage, transform, vote (chunked)
+        for (int cbeg = 0; cbeg < n; cbeg += p.chunk) {
+            const int m = min(p.chunk, n - cbeg);
+            int tame = 1;
+            for (int i = tid; i < m; i += nthreads) {
+                float2 h = __ldg(&p.xy[beg + cbeg + i]);
+                float2 uv = conformal(h, p.scale);
+                hb[i] = uv;
+                tame &= (__fadd_rn(fabsf(uv.x), fabsf(uv.y)) <= p.tame_bound) ? 1 : 0;   // false for NaN/inf
+            }
+            const int all_tame = __shfl_sync(0xffffffffu, __syncthreads_and(tame) && !p.force_slow, 0);
+            // Every warp votes (nwarps == n_groups * n_stripes).  Hits are dealt in rounds of 4*S:
+            // the full rounds have a warp-uniform trip count, which keeps the loop in uniform
+            // control flow (shared-window base in a uniform register, ATOMS [R+UR] addressing).
+            const int S = p.n_stripes;
+            const int R = m / (4 * S);
+            if (all_tame) {
+                for (int r = 0; r < R; ++r) {
+                    float2 uv[4];
+#pragma unroll
+                    for (int q = 0; q < 4; ++q) uv[q] = hb[(4 * r + q) * S + stripe];
+#pragma unroll
+                    for (int q = 0; q < 4; ++q) {
+                        const unsigned b0 = bin_bits(uv[q].x, uv[q].y, c0, s0, rho_max, inv);
+                        const unsigned b1 = bin_bits(uv[q].x, uv[q].y, c1, s1, rho_max, inv);
+                        // out-of-range votes (rel >= limit, including every wrapped negative) land in the
+                        // lane's own word of the trash row n_rho: no predicate, no branch, no conflict
+                        const unsigned rel0 = min(b0 * pitch + lc0, trash0);
+                        const unsigned rel1 = min(b1 * pitch + lc1, trash1);
+                        atomicAdd((unsigned*)(acc + rel0), inc0);
+                        atomicAdd((unsigned*)(acc + rel1), inc1);
+                    }
+                }
+                for (int i = 4 * R * S + stripe; i < m; i += S) {
+                    const float2 uv = hb[i];
+                    const unsigned b0 = bin_bits(uv.x, uv.y, c0, s0, rho_max, inv);
+                    const unsigned b1 = bin_bits(uv.x, uv.y, c1, s1, rho_max, inv);
+                    const unsigned rel0 = min(b0 * pitch + lc0, trash0);
+                    const unsigned rel1 = min(b1 * pitch + lc1, trash1);
+                    atomicAdd((unsigned*)(acc + rel0), inc0);
+                    atomicAdd((unsigned*)(acc + rel1), inc1);
+                }
+            } else {
+                // exact slow path: literal S2 with float compares (degenerate hits: NaN, inf, r < ~0.3 mm)
+                for (int i = stripe; i < m; i += S) {
+                    const float2 uv = hb[i];
+                    int k0 = bin_exact(uv.x, uv.y, c0, s0, p.rho_max, p.inv, p.n_rho);
+                    int k1 = bin_exact(uv.x, uv.y, c1, s1, p.rho_max, p.inv, p.n_rho);
+                    if (valid0 && k0 >= 0) red_shared_add(acc_s + (unsigned)k0 * pitch + woff0, inc0);
+                    if (valid1 && k1 >= 0) red_shared_add(acc_s + (unsigned)k1 * pitch + woff1, inc1);
+                }
+            }
+            __syncthreads();
+        }
+        if (CL) cg::this_cluster().sync();   // (A) every CTA's columns are complete
+
+        // ---- optional accumulator dump (parity / debugging; never timed)
+        if (p.accum_dump) {
+            unsigned* dst = p.accum_dump + ((size_t)e * p.n_theta + col0) * p.n_rho;
+            const int cells = ncols * p.n_rho;
+            for (int idx = tid; idx < cells; idx += nthreads) {
+                int jl = idx / p.n_rho, k = idx - jl * p.n_rho;
+                dst[idx] = cell_from<ACC16>(acc, p.pitch_b, jl, k);
+            }
+        }
+
+        // ---- H4: threshold + 3x3 local maximum -> peak bitmap (reading Q8)
+        {
+            auto cell_global = [&](int j, int k) -> unsigned {
+                if (j < 0 || j >= p.n_theta || k < 0 || k >= p.n_rho) return 0u;   // outside = 0, no theta wrap
+                int owner = j / p.cols_per_cta;
+                int jl = j - owner * p.cols_per_cta;
+                if (!CL || owner == (int)rank) return cell_from<ACC16>(acc, p.pitch_b, jl, k);
+                const unsigned char* racc = (const unsigned char*)cg::this_cluster().map_shared_rank((void*)acc, owner);
+                return cell_from<ACC16>(racc, p.pitch_b, jl, k);
+            };
+            auto test_peak = [&](int jl, int k, unsigned a) {
+                const int j = col0 + jl;
+                bool ok = true;
+#pragma unroll
+                for (int dj = -1; dj <= 1; ++dj) {
+#pragma unroll
+                    for (int dk = -1; dk <= 1; ++dk) {
+                        if (dj == 0 && dk == 0) continue;
+                        const unsigned nb = cell_global(j + dj, k + dk);
+                        const bool precedes = (dj < 0) || (dj == 0 && dk < 0);
+                        ok = ok && (precedes ? (a > nb) : (a >= nb));
+                    }
+                }
+                if (ok) red_shared_or((unsigned)__cvta_generic_to_shared(&pbm[jl * p.wpr + (k >> 5)]), 1u << (k & 31));
+            };
+            const int nwg = p.pitch_b >> 7;                 // word groups (32 words) per rho row
+            const int items = p.n_rho * nwg;
+            const unsigned thr = (unsigned)p.threshold;
+            for (int it = warp; it < items; it += nwarps) {
+                const int k = it / nwg, wg = it - k * nwg;
+                const unsigned w = *(const unsigned*)(acc + (size_t)k * p.pitch_b + 4u * (wg * 32 + lane));
+                if (ACC16) {
+                    const unsigned a0 = w & 0xFFFFu, a1 = w >> 16;
+                    if (a0 >= thr) test_peak(64 * wg + lane, k, a0);
+                    if (a1 >= thr) test_peak(64 * wg + 32 + lane, k, a1);
+                } else {
+                    if (w >= thr) test_peak(32 * wg + lane, k, w);   // 32*wg + lane == 64*(wg>>1) + 32*(wg&1) + lane
+                }
+            }
+        }
+        __syncthreads();
+
+        // ---- H5: raster-order peak list.  pbm is [jl][k/32]: ascending word index is raster order.
+        const int W = ncols * p.wpr;
+        const int span = (W + nthreads - 1) / nthreads;
+        const int w_lo = min(tid * span, W), w_hi = min(w_lo + span, W);
+        int my_peaks = 0;
+        for (int w = w_lo; w < w_hi; ++w) my_peaks += __popc(pbm[w]);
+        int cta_peaks;
+        int pos = block_exscan(my_peaks, misc, cta_peaks);
+        int base = 0, n_peaks = cta_peaks;
+        if (CL) {
+            if (tid == 0) misc[40] = cta_peaks;
+            cg::this_cluster().sync();   // (B) all scans done (accumulators no longer read remotely); totals visible
+            n_peaks = 0;
+            for (int r = 0; r < C; ++r) {
+                int t = *(const int*)cg::this_cluster().map_shared_rank((void*)&misc[40], r);
+                if (r < (int)rank) base += t;
+                n_peaks += t;
+            }
+        }
+        pos += base;
+        for (int w = w_lo; w < w_hi && pos < p.max_peaks; ++w) {
+            unsigned bits = pbm[w];
+            const int jl = w / p.wpr, kb = (w - jl * p.wpr) << 5;
+            while (bits && pos < p.max_peaks) {
+                const int k = kb + __ffs(bits) - 1;
+                bits &= bits - 1;
+                hough_peak pk;
+                pk.theta_bin = (uint16_t)(col0 + jl);
+                pk.rho_bin = (uint16_t)k;
+                pk.votes = cell_from<ACC16>(acc, p.pitch_b, jl, k);
+                p.peaks[(size_t)e * p.max_peaks + pos] = pk;
+                ++pos;
+            }
+        }
+        if (rank == 0 && tid == 0) p.counts[2 * e] = n_peaks;
+        const int n_stored = min(n_peaks, p.max_peaks);
+        if (CL) {
+            __threadfence();
+            cg::this_cluster().sync();   // (C) stored peaks visible cluster-wide; accumulator region is dead
+        } else {
+            __syncthreads();
+        }
+
+        // ---- H6 set-up: dilated bitmap D[n_theta+1][wpr] (union of the stored peaks' windows; row n_theta = zero dummy)
+        unsigned* D = (unsigned*)(acc + p.d_off);
+        float* mcf = (float*)(acc + p.mcf_off);
+        float* msf = (float*)(acc + p.msf_off);
+        int* mrow = (int*)(acc + p.mrow_off);
+        const int d_words = (p.n_theta + 1) * p.wpr;
+        for (int i = tid; i < d_words; i += nthreads) D[i] = 0u;
+        if (tid == 0) misc[41] = 0;
+        __syncthreads();
+        for (int q = tid; q < n_stored; q += nthreads) {
+            const hough_peak pk = p.peaks[(size_t)e * p.max_peaks + q];
+            const int jlo = max(0, (int)pk.theta_bin - p.window), jhi = min(p.n_theta - 1, (int)pk.theta_bin + p.window);
+            const int klo = max(0, (int)pk.rho_bin - p.window), khi = min(p.n_rho - 1, (int)pk.rho_bin + p.window);
+            for (int j = jlo; j <= jhi; ++j) {
+                for (int wd = klo >> 5; wd <= khi >> 5; ++wd) {
+                    const int a = max(klo, wd << 5) & 31, b = min(khi, (wd << 5) + 31) & 31;
+                    const unsigned mask = (0xFFFFFFFFu >> (31 - b)) & (0xFFFFFFFFu << a);
+                    red_shared_or((unsigned)__cvta_generic_to_shared(&D[j * p.wpr + wd]), mask);
+                }
+            }
+        }
+        __syncthreads();
+        // marked columns: those with any bit set (order irrelevant for the OR below)
+        for (int jb = 0; jb < p.n_theta; jb += nthreads) {
+            const int j = jb + tid;
+            bool any = false;
+            if (j < p.n_theta) {
+                unsigned o = 0;
+                for (int wd = 0; wd < p.wpr; ++wd) o |= D[j * p.wpr + wd];
+                any = o != 0u;
+            }
+            const unsigned bal = __ballot_sync(0xffffffffu, any);
+            int wbase = 0;
+            if (lane == 0 && bal) wbase = atomicAdd(&misc[41], __popc(bal));
+            wbase = __shfl_sync(0xffffffffu, wbase, 0);
+            if (any) {
+                const int q = wbase + __popc(bal & ((1u << lane) - 1u));
+                mcf[q] = p.cos_t[j];
+                msf[q] = p.sin_t[j];
+                mrow[q] = j * p.wpr;
+            }
+        }
+        __syncthreads();
+        int n_marked = misc[41];
+        if (n_marked & 1) {   // pad to a pair with a column that can never keep (zero dummy row)
+            if (tid == 0) { mcf[n_marked] = 0.0f; msf[n_marked] = 0.0f; mrow[n_marked] = p.n_theta * p.wpr; }
+            ++n_marked;
+        }
+        __syncthreads();
+
+        // keep test of one hit: OR over marked columns of D[j][bin(i,j)]  (== S5)
+        auto keep_test = [&](float2 uv, bool valid) -> bool {
+            bool kp = false;
+            for (int mq = 0; mq < n_marked; mq += 2) {
+                const float2 mc = *(const float2*)(mcf + mq), ms = *(const float2*)(msf + mq);
+                const int2 rows = *(const int2*)(mrow + mq);
+                const unsigned k0 = bin_bits(uv.x, uv.y, mc.x, ms.x, rho_max, inv) - HOUGH_MAGIC_BITS;
+                const unsigned k1 = bin_bits(uv.x, uv.y, mc.y, ms.y, rho_max, inv) - HOUGH_MAGIC_BITS;
+                if (k0 < (unsigned)p.n_rho) kp = kp || ((D[rows.x + (k0 >> 5)] >> (k0 & 31)) & 1u);
+                if (k1 < (unsigned)p.n_rho) kp = kp || ((D[rows.y + (k1 >> 5)] >> (k1 & 31)) & 1u);
+                if ((mq & 6) == 6 && __all_sync(0xffffffffu, kp || !valid)) break;
+            }
+            return kp && valid;
+        };
+
+        // ---- H6 + H7
+        if (!CL) {
+            int kept_base = 0;
+            for (int b0i = 0; b0i < n; b0i += nthreads) {
+                const int i = b0i + tid;
+                const bool valid = i < n;
+                float2 h = make_float2(1.0f, 0.0f);
+                if (valid) h = __ldg(&p.xy[beg + i]);
+                const bool kp = keep_test(conformal(h, p.scale), valid);
+                int blk_total;
+                const int ppos = block_exscan(kp ? 1 : 0, misc, blk_total);
+                if (valid) {
+                    p.keep[beg + i] = kp ? 1 : 0;
+                    if (kp) {
+                        if (p.kept_xy) p.kept_xy[beg + kept_base + ppos] = h;
+                        if (p.kept_idx) p.kept_idx[beg + kept_base + ppos] = i;
+                    }
+                }
+                kept_base += blk_total;
+            }
+            if (tid == 0) p.counts[2 * e + 1] = kept_base;
+            __syncthreads();   // D / lists are dead: the region may be zeroed for the next event
+        } else {
+            // clustered: hit blocks are dealt round-robin to the CTAs; two passes per round
+            unsigned* stash = (unsigned*)(acc + p.stash_off);   // [round block][warp] ballots
+            int* cnt = (int*)(acc + p.cnt_off);                 // my blocks' kept counts (remote-readable)
+            int* gcnt = (int*)(acc + p.gcnt_off);               // exclusive bases of this round's blocks
+            const int n_blocks = (n + nthreads - 1) / nthreads;
+            const int round_blocks = HOUGH_SEL_ROUND_BLOCKS * C;
+            int kept_base = 0;
+            for (int rb = 0; rb < n_blocks; rb += round_blocks) {
+                const int rnb = min(round_blocks, n_blocks - rb);
+                for (int bl = 0; rb + bl * C + (int)rank < rb + rnb; ++bl) {
+                    const int i = (rb + bl * C + (int)rank) * nthreads + tid;
+                    const bool valid = i < n;
+                    float2 h = make_float2(1.0f, 0.0f);
+                    if (valid) h = __ldg(&p.xy[beg + i]);
+                    const bool kp = keep_test(conformal(h, p.scale), valid);
+                    const unsigned bal = __ballot_sync(0xffffffffu, kp);
+                    if (lane == 0) stash[bl * nwarps + warp] = bal;
+                    if (valid) p.keep[beg + i] = kp ? 1 : 0;
+                    const int tot = __syncthreads_count(kp);
+                    if (tid == 0) cnt[bl] = tot;
+                }
+                cg::this_cluster().sync();   // (D) counts of this round visible
+                // exclusive bases of the round's blocks (every CTA computes all; tiny)
+                if (warp == 0) {
+                    int run = kept_base;
+                    for (int b = 0; b < rnb; b += 32) {
+                        const int bb = b + lane;
+                        int v = 0;
+                        if (bb < rnb) v = *(const int*)cg::this_cluster().map_shared_rank((void*)&cnt[bb / C], bb % C);
+                        int incl = v;
+#pragma unroll
+                        for (int d = 1; d < 32; d <<= 1) {
+                            int o = __shfl_up_sync(0xffffffffu, incl, d);
+                            if (lane >= d) incl += o;
+                        }
+                        if (bb < rnb) gcnt[bb] = run + incl - v;
+                        run += __shfl_sync(0xffffffffu, incl, 31);
+                    }
+                    if (lane == 0) gcnt[rnb] = run;
+                }
+                __syncthreads();
+                for (int bl = 0; rb + bl * C + (int)rank < rb + rnb; ++bl) {
+                    const int bb = bl * C + (int)rank;
+                    const int i = (rb + bb) * nthreads + tid;
+                    const unsigned bal = stash[bl * nwarps + warp];
+                    if ((bal >> lane) & 1u) {
+                        int ppos = gcnt[bb] + __popc(bal & ((1u << lane) - 1u));
+                        for (int w2 = 0; w2 < warp; ++w2) ppos += __popc(stash[bl * nwarps + w2]);
+                        if (p.kept_xy) p.kept_xy[beg + ppos] = __ldg(&p.xy[beg + i]);
+                        if (p.kept_idx) p.kept_idx[beg + ppos] = i;
+                    }
+                }
+                kept_base = gcnt[rnb];
+                cg::this_cluster().sync();   // (E) remote reads of cnt done before it is rewritten / zeroed
+            }
+            if (rank == 0 && tid == 0) p.counts[2 * e + 1] = kept_base;
+        }
+    }
+}
+
+}  // namespace hough

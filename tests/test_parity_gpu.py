@@ -1,0 +1,345 @@
+"""-m gpu: the CUDA path, called through the C ABI, against the CPU oracle,
+element by element and bit for bit (accumulators, peak lists, counts, keep
+masks, compacted order) on the same seeded inputs."""
+import numpy as np
+import pytest
+
+import oracle
+import stcf_inputs as si
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def hb():
+    import torch
+    assert torch.cuda.is_available()
+    import paper_2607_04067_b200 as m
+    m.load_library()
+    return m
+
+
+def gpu_run(hb, xy, off, n_theta, n_rho, rho_max, threshold, window, table, max_peaks=64, acc_dtype="u16",
+            accum=True, conformal_scale=1, cluster_size=0, ctas_per_sm=0, vote_path=0, stream=None):
+    import torch
+    h = hb.Hough(n_theta, n_rho, rho_max, threshold, window, max_peaks=max_peaks, acc_dtype=acc_dtype,
+                 conformal_scale=conformal_scale, cluster_size=cluster_size, ctas_per_sm=ctas_per_sm, trig_table=table)
+    try:
+        if vote_path:
+            hb.hough_set_option(h.ctx, hb.HOUGH_OPT_VOTE_PATH, vote_path)
+        d_xy = torch.from_numpy(np.ascontiguousarray(xy, dtype=np.float32).reshape(-1, 2)).cuda()
+        d_off = torch.from_numpy(np.ascontiguousarray(off, dtype=np.int32)).cuda()
+        # poison the outputs so that "untouched" and "written" are distinguishable
+        out = h.alloc_outputs(d_xy.shape[0], d_off.numel() - 1, accum=accum)
+        out["keep"].fill_(7)
+        out["counts"].fill_(-99)
+        out["kept_idx"].fill_(-5)
+        out["peaks"].fill_(-1)
+        h.run(d_xy, d_off, out=out, stream=stream)
+        torch.cuda.synchronize()
+        res = {k: v.cpu().numpy() for k, v in out.items()}
+        res["peaks3"] = hb.unpack_peaks(res["peaks"])
+        res["info"] = {k: h.info(getattr(hb, "HOUGH_INFO_" + k)) for k in
+                       ("CLUSTER_SIZE", "THREADS", "SMEM_BYTES", "CTAS_PER_SM", "GRID_MAX", "ACC_BITS", "CHUNK_HITS")}
+        return res
+    finally:
+        h.close()
+
+
+def compare(g, o, off, max_peaks, accum=True, tag=""):
+    n_events = len(off) - 1
+    assert np.array_equal(g["counts"], o.counts), tag + " counts"
+    if accum:
+        assert np.array_equal(g["accum"].view(np.uint32), o.accum), tag + " accumulator"
+    for e in range(n_events):
+        if o.counts[e, 0] < 0:
+            continue
+        ns = min(int(o.counts[e, 0]), max_peaks)
+        assert np.array_equal(g["peaks3"][e, :ns], o.peaks[e, :ns]), "%s peaks of event %d" % (tag, e)
+        # entries past the stored ones are untouched (poison = all ones)
+        if ns < max_peaks:
+            assert np.all(g["peaks"][e, ns:] == -1), "%s peak tail of event %d" % (tag, e)
+        nk = int(o.counts[e, 1])
+        a = int(off[e])
+        assert np.array_equal(g["kept_idx"][a:a + nk], o.kept_idx[a:a + nk]), "%s kept_idx of event %d" % (tag, e)
+        assert np.array_equal(g["kept_xy"][a:a + nk].view(np.uint32), o.kept_xy[a:a + nk].view(np.uint32)), tag
+        assert np.all(g["kept_idx"][a + nk:int(off[e + 1])] == -5), "%s kept tail of event %d" % (tag, e)
+    ok_ev = o.counts[:, 0] >= 0
+    mask = np.repeat(ok_ev, np.diff(off))
+    assert np.array_equal(g["keep"][mask], o.keep[mask]), tag + " keep mask"
+
+
+def run_both(hb, w, xy, off, accum=True, **kw):
+    table = si.trig_table(w.n_theta)
+    args = dict(max_peaks=w.max_peaks, acc_dtype=w.acc_dtype, threshold=w.threshold, window=w.window)
+    args.update(kw)
+    gpu_only = {k: args.pop(k) for k in ("cluster_size", "ctas_per_sm", "vote_path") if k in args}
+    g = gpu_run(hb, xy, off, w.n_theta, w.n_rho, w.rho_max, args["threshold"], args["window"], table,
+                max_peaks=args["max_peaks"], acc_dtype=args["acc_dtype"], accum=accum,
+                conformal_scale=args.get("conformal_scale", 1), **gpu_only)
+    o = oracle.run(xy, off, w.n_theta, w.n_rho, w.rho_max, args["threshold"], args["window"], table[0], table[1],
+                   max_peaks=args["max_peaks"], conformal_scale=args.get("conformal_scale", 1),
+                   acc_u16=(args["acc_dtype"] != "u32"), want_accum=accum, n_threads=8)
+    compare(g, o, off, args["max_peaks"], accum=accum, tag=w.name)
+    return g, o
+
+
+# ---------------------------------------------------------------- paper-pinned cases through the CUDA path
+def test_w1_worked_example_on_gpu(hb):
+    xy = np.array([[1, 0], [0, 1], [.5, .5], [-1, 0], [0, 0], [4, 0]], dtype=np.float32)
+    off = np.array([0, 6], dtype=np.int32)
+    table = si.trig_table(4)
+    for thr, w, exp_keep in ((2, 0, [1, 1, 1, 1, 0, 1]), (3, 0, [1, 0, 0, 1, 0, 1]), (3, 1, [1, 1, 1, 1, 0, 1])):
+        g = gpu_run(hb, xy, off, 4, 8, 2.0, thr, w, table, max_peaks=8)
+        o = oracle.run(xy, off, 4, 8, 2.0, thr, w, table[0], table[1], max_peaks=8, want_accum=True)
+        compare(g, o, off, 8, tag="W1")
+        assert g["keep"].tolist() == exp_keep
+    assert g["accum"][0].tolist() == [[0, 0, 1, 0, 2, 0, 2, 0], [0, 0, 1, 0, 1, 2, 1, 0],
+                                      [0, 0, 0, 0, 3, 0, 2, 0], [0, 0, 1, 1, 1, 2, 0, 0]]
+
+
+def test_p1_closed_form_on_gpu(hb):
+    nt, nr, jstar, kstar = 180, 128, 40, 70
+    inv = 21376.0
+    R = 1.0 / (2.0 * ((kstar + 0.5) / inv - float(si.RHO_MAX)))
+    r = 200.0 + np.arange(48) * 600.0 / 47.0
+    phi = jstar * np.pi / nt - np.arccos(r / (2 * R))
+    xy = np.stack([r * np.cos(phi), r * np.sin(phi)], axis=1).astype(np.float32)
+    off = np.array([0, 48], dtype=np.int32)
+    g = gpu_run(hb, xy, off, nt, nr, si.RHO_MAX, 20, 1, si.trig_table(nt))
+    A = g["accum"][0]
+    assert A[jstar, kstar] == 48 and np.count_nonzero(A[jstar]) == 1 and int(A.sum()) == 7853
+    assert [jstar, kstar, 48] in g["peaks3"][0, :g["counts"][0, 0]].tolist()
+    assert g["keep"].all()
+
+
+# ---------------------------------------------------------------- the five configurations
+@pytest.mark.parametrize("cfg,n_ev", [(0, 16), (1, 96), (2, 48), (3, 24)])
+def test_configs_with_accumulator(hb, cfg, n_ev):
+    w = si.config(cfg)
+    xy, off, _ = si.generate(w, n_ev)
+    run_both(hb, w, xy, off)
+
+
+@pytest.mark.parametrize("cfg", [1, 2, 3])
+def test_configs_full_batch_1000_events(hb, cfg):
+    # BASELINE.json sizes, in the launch configuration bench.py times (no accumulator dump)
+    w = si.config(cfg)
+    xy, off, _ = si.generate(w)
+    g, o = run_both(hb, w, xy, off, accum=False)
+    assert g["info"]["CLUSTER_SIZE"] == 1
+
+
+def test_cfg4_cluster_grid_360x512(hb):
+    w = si.config(5)
+    xy, off, _ = si.generate(w, 64)
+    g, _ = run_both(hb, w, xy, off)
+    assert g["info"]["CLUSTER_SIZE"] >= 2     # the 360 KB accumulator cannot live in one SM
+
+
+def test_cfg4_sweep_sampled_parity_100k(hb):
+    # all 100k events through the GPU; the oracle checks a sample of whole events plus global invariants
+    w = si.config(4)
+    xy, off, _ = si.generate(w)
+    table = si.trig_table(w.n_theta)
+    g = gpu_run(hb, xy, off, w.n_theta, w.n_rho, w.rho_max, w.threshold, w.window, table, accum=False)
+    n = np.diff(off)
+    assert np.all(g["counts"][:, 1] >= 0) and np.all(g["counts"][:, 1] <= n) and np.all(g["counts"][:, 0] >= 0)
+    kept_per_event = np.add.reduceat(g["keep"].astype(np.int64), off[:-1])
+    assert np.array_equal(kept_per_event, g["counts"][:, 1])
+    rng = np.random.default_rng(11)
+    for e0 in rng.choice(len(n) - 50, size=12, replace=False):
+        sl = slice(int(off[e0]), int(off[e0 + 50]))
+        o = oracle.run(xy[sl], off[e0:e0 + 51] - off[e0], w.n_theta, w.n_rho, w.rho_max, w.threshold, w.window,
+                       table[0], table[1], max_peaks=w.max_peaks, n_threads=8)
+        assert np.array_equal(g["counts"][e0:e0 + 50], o.counts)
+        assert np.array_equal(g["keep"][sl], o.keep)
+        for i in range(50):
+            ns = min(int(o.counts[i, 0]), w.max_peaks)
+            assert np.array_equal(g["peaks3"][e0 + i, :ns], o.peaks[i, :ns])
+            nk, a = int(o.counts[i, 1]), int(off[e0 + i])
+            assert np.array_equal(g["kept_idx"][a:a + nk], o.kept_idx[a - sl.start:a - sl.start + nk])
+
+
+# ---------------------------------------------------------------- variants of the launch
+@pytest.mark.parametrize("cluster", [2, 4])
+def test_forced_cluster_matches_oracle(hb, cluster):
+    w = si.config(1)
+    xy, off, _ = si.generate(w, 40)
+    g, _ = run_both(hb, w, xy, off, cluster_size=cluster)
+    assert g["info"]["CLUSTER_SIZE"] == cluster
+
+
+def test_one_cta_per_sm_and_slow_vote_path(hb):
+    w = si.config(0)
+    xy, off, _ = si.generate(w)
+    run_both(hb, w, xy, off, ctas_per_sm=1)
+    run_both(hb, w, xy, off, vote_path=1)
+
+
+@pytest.mark.parametrize("window", [0, 2, 5])
+def test_windows(hb, window):
+    w = si.config(1)
+    xy, off, _ = si.generate(w, 24)
+    run_both(hb, w, xy, off, window=window)
+
+
+@pytest.mark.parametrize("max_peaks", [0, 1, 3, 4096])
+def test_max_peaks_truncation(hb, max_peaks):
+    w = si.config(2)        # hundreds of peaks per event
+    xy, off, _ = si.generate(w, 12)
+    g, o = run_both(hb, w, xy, off, max_peaks=max_peaks)
+    assert o.counts[:, 0].max() > 64
+
+
+def test_conformal_scale_2(hb):
+    w = si.config(0)
+    xy, off, _ = si.generate(w, 8)
+    table = si.trig_table(w.n_theta)
+    g1 = gpu_run(hb, xy, off, w.n_theta, w.n_rho, w.rho_max, w.threshold, w.window, table)
+    g2 = gpu_run(hb, xy, off, w.n_theta, w.n_rho, np.float32(2) * np.float32(w.rho_max), w.threshold, w.window,
+                 table, conformal_scale=2)
+    for k in ("accum", "counts", "keep", "kept_idx", "peaks"):
+        assert np.array_equal(g1[k], g2[k]), k          # pin P5 on the GPU
+
+
+# ---------------------------------------------------------------- edge cases
+def test_empty_and_ragged_events(hb):
+    w = si.config(0)
+    xy, off, _ = si.generate(w, 6)
+    off2 = np.concatenate([[0, 0], off[1:4], [off[3], off[3]], off[4:], [off[-1]]]).astype(np.int32)
+    run_both(hb, w, xy, off2)
+    # single-hit and two-hit events, threshold 1: every hit is its own peak neighbourhood
+    xy1 = np.array([[300, 0], [0, 450], [200, 200], [-700, 100]], dtype=np.float32)
+    off1 = np.array([0, 1, 3, 3, 4], dtype=np.int32)
+    run_both(hb, w, xy1, off1, threshold=1, max_peaks=512)
+    # all events empty
+    g = gpu_run(hb, xy[:0], np.zeros(5, dtype=np.int32), w.n_theta, w.n_rho, w.rho_max, 20, 1, si.trig_table(w.n_theta))
+    assert not g["counts"].any()
+
+
+def test_degenerate_hits_take_the_exact_slow_path(hb):
+    # NaN (0,0), inf, tiny radii (|t| huge), denormals: literal S2 semantics (reading Q5)
+    w = si.config(0)
+    xy, off, _ = si.generate(w, 3)
+    bad = np.array([[0, 0], [np.inf, 1], [1e-3, 0], [0, -1e-3], [1e-20, 1e-20], [np.nan, 5], [1e-30, 0],
+                    [1e30, 1e30], [-1e-3, 1e-3], [3e38, 0]], dtype=np.float32)
+    xy2 = np.concatenate([xy[:off[1]], bad, xy[off[1]:]])
+    off2 = off.copy()
+    off2[1:] += len(bad)
+    g, o = run_both(hb, w, xy2, off2, threshold=5)
+    assert o.accum[0].sum() > 0
+
+
+def test_event_larger_than_the_staging_chunk(hb):
+    w = si.config(3)
+    xy, off, _ = si.generate(w, 6)
+    big = np.concatenate([xy[:off[6]]])                 # ~17000 hits as ONE event
+    off_big = np.array([0, len(big)], dtype=np.int32)
+    g, _ = run_both(hb, w, big, off_big, threshold=60)
+    assert g["info"]["CHUNK_HITS"] < len(big)
+    g, _ = run_both(hb, si.config(1), big, off_big, threshold=60)   # u16, two CTAs per SM
+
+
+def test_u16_overflow_event_is_refused(hb):
+    n = 65536
+    rng = np.random.default_rng(3)
+    phi = rng.uniform(0, 2 * np.pi, n)
+    xy = np.stack([400 * np.cos(phi), 400 * np.sin(phi)], axis=1).astype(np.float32)
+    xy = np.concatenate([xy, np.array([[300, 0], [0, 300], [250, 250]], dtype=np.float32)])
+    off = np.array([0, n, n + 3], dtype=np.int32)
+    w = si.config(0)
+    table = si.trig_table(w.n_theta)
+    g = gpu_run(hb, xy, off, w.n_theta, w.n_rho, w.rho_max, 1, 0, table, accum=False)
+    assert g["counts"][0].tolist() == [-1, -1]
+    assert np.all(g["keep"][:n] == 7)                    # nothing else written for the refused event
+    o = oracle.run(xy, off, w.n_theta, w.n_rho, w.rho_max, 1, 0, table[0], table[1])
+    assert np.array_equal(g["counts"], o.counts) and np.array_equal(g["keep"][n:], o.keep[n:])
+    # the same event under a u32 accumulator is processed
+    run_both(hb, w, xy, off, threshold=400, acc_dtype="u32", accum=False)
+
+
+def test_tiny_and_odd_grids(hb):
+    w = si.config(0)
+    xy, off, _ = si.generate(w, 4)
+    for nt, nr in ((1, 1), (3, 5), (33, 31), (65, 100), (130, 257), (200, 40)):
+        table = si.trig_table(nt)
+        g = gpu_run(hb, xy, off, nt, nr, w.rho_max, 4, 1, table, max_peaks=256)
+        o = oracle.run(xy, off, nt, nr, w.rho_max, 4, 1, table[0], table[1], max_peaks=256, want_accum=True)
+        compare(g, o, off, 256, tag="%dx%d" % (nt, nr))
+
+
+# ---------------------------------------------------------------- API behaviour
+def test_plain_hough_run_and_streams_and_reentrancy(hb):
+    import torch
+    w = si.config(1)
+    xy, off, _ = si.generate(w, 60)
+    table = si.trig_table(w.n_theta)
+    o = oracle.run(xy, off, w.n_theta, w.n_rho, w.rho_max, w.threshold, w.window, table[0], table[1], max_peaks=w.max_peaks)
+    h = hb.Hough(w.n_theta, w.n_rho, w.rho_max, w.threshold, w.window, trig_table=table)
+    d_xy, d_off = torch.from_numpy(xy).cuda(), torch.from_numpy(off).cuda()
+    outs, streams = [], [torch.cuda.Stream() for _ in range(3)]
+    torch.cuda.synchronize()
+    for s in streams:      # the same handle on three streams at once: no per-run scratch
+        keep = torch.empty(len(xy), dtype=torch.uint8, device="cuda")
+        peaks = torch.zeros((60, 64, 2), dtype=torch.int32, device="cuda")
+        counts = torch.empty((60, 2), dtype=torch.int32, device="cuda")
+        hb.hough_run(h.ctx, d_xy, d_off, 60, keep, peaks, counts, stream=s)
+        outs.append((keep, peaks, counts))
+    torch.cuda.synchronize()
+    for keep, peaks, counts in outs:
+        assert np.array_equal(counts.cpu().numpy(), o.counts)
+        assert np.array_equal(keep.cpu().numpy(), o.keep)
+    assert h.info(hb.HOUGH_INFO_LAUNCHES) == 3
+    # n_events == 0 is a no-op; bad arguments are refused
+    hb.hough_run(h.ctx, d_xy, d_off, 0, keep, peaks, counts)
+    with pytest.raises(hb.HoughError):
+        hb.hough_run(h.ctx, None, d_off, 60, keep, peaks, counts)
+    with pytest.raises(hb.HoughError):
+        hb.hough_set_option(h.ctx, hb.HOUGH_OPT_CLUSTER_SIZE, 3)
+    h.close()
+    with pytest.raises(hb.HoughError):
+        hb.hough_create(0, 10, 1.0, 1, 0)
+    with pytest.raises(hb.HoughError):
+        hb.Hough(1000, 1000, 0.01, 10, 1)            # the paper's own grid: NEXT-3, does not fit a cluster yet
+
+
+def test_run_host_end_to_end(hb):
+    import torch
+    w = si.config(1)
+    xy, off, _ = si.generate(w, 80)
+    table = si.trig_table(w.n_theta)
+    o = oracle.run(xy, off, w.n_theta, w.n_rho, w.rho_max, w.threshold, w.window, table[0], table[1], max_peaks=w.max_peaks)
+    h = hb.Hough(w.n_theta, w.n_rho, w.rho_max, w.threshold, w.window, trig_table=table)
+    h_xy = torch.from_numpy(xy).pin_memory()
+    h_off = torch.from_numpy(off).pin_memory()
+    keep = torch.empty(len(xy), dtype=torch.uint8).pin_memory()
+    peaks = torch.zeros((80, 64, 2), dtype=torch.int32).pin_memory()
+    counts = torch.empty((80, 2), dtype=torch.int32).pin_memory()
+    kept_xy = torch.zeros((len(xy), 2), dtype=torch.float32).pin_memory()
+    kept_idx = torch.zeros(len(xy), dtype=torch.int32).pin_memory()
+    for _ in range(2):
+        hb.hough_run_host(h.ctx, h_xy, h_off, 80, keep, peaks, counts, kept_xy, kept_idx)
+        torch.cuda.synchronize()
+        assert np.array_equal(counts.numpy(), o.counts) and np.array_equal(keep.numpy(), o.keep)
+        p3 = hb.unpack_peaks(peaks.numpy())
+        for e in range(80):
+            ns = min(int(o.counts[e, 0]), 64)
+            assert np.array_equal(p3[e, :ns], o.peaks[e, :ns])
+            nk, a = int(o.counts[e, 1]), int(off[e])
+            assert np.array_equal(kept_idx.numpy()[a:a + nk], o.kept_idx[a:a + nk])
+    h.close()
+
+
+def test_default_trig_table_equals_harness_table(hb):
+    w = si.config(0)
+    xy, off, _ = si.generate(w, 4)
+    table = si.trig_table(w.n_theta)
+    a = gpu_run(hb, xy, off, w.n_theta, w.n_rho, w.rho_max, w.threshold, w.window, table)
+    b = gpu_run(hb, xy, off, w.n_theta, w.n_rho, w.rho_max, w.threshold, w.window, None)
+    assert np.array_equal(a["accum"], b["accum"]) and np.array_equal(a["keep"], b["keep"])
+
+
+def test_shared_atomic_microbench_runs(hb):
+    r = hb.hough_bench_shared_atomics(0, 2, 512, 2000)
+    assert r > 1e11

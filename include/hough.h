@@ -169,6 +169,8 @@ const char* hough_version(void);
  *   variant 2: pseudo-random bank per lane (natural bank conflicts)
  *   variant 3: the voting loop's instruction mix without the atomics (issue bound)
  *   variant 4: the voting loop's instruction mix with conflict-free atomics
+ *   variant 5: the ATOMS pipe alone: eight fixed conflict-free addresses per thread, no address
+ *              arithmetic in the loop (the peak the vote roofline divides by)
  * Synchronises the device. */
 int hough_bench_shared_atomics(int variant, int ctas_per_sm, int threads, long long iters, double* out_rate);
 

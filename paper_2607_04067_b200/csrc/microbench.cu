@@ -41,6 +41,26 @@ __global__ void __launch_bounds__(1024, 1) atomics_kernel(long long iters, unsig
     if (sink && threadIdx.x == 0) sink[blockIdx.x] = a[lane];
 }
 
+// variant 5: the ATOMS pipe alone -- eight fixed, conflict-free addresses per thread (lane == bank), no address
+// arithmetic in the loop.  This is the denominator of the vote roofline.
+__global__ void __launch_bounds__(1024, 1) atomics_peak_kernel(long long iters, unsigned* sink) {
+    extern __shared__ __align__(128) unsigned char smem[];
+    unsigned* a = (unsigned*)smem;
+    for (int i = threadIdx.x; i < 8192; i += blockDim.x) a[i] = 0;
+    __syncthreads();
+    const unsigned s = (unsigned)__cvta_generic_to_shared(a) + (threadIdx.x & 31) * 4u;
+    const unsigned a0 = s, a1 = s + 128 * 3, a2 = s + 128 * 7, a3 = s + 128 * 12, a4 = s + 128 * 17, a5 = s + 128 * 21,
+                   a6 = s + 128 * 30, a7 = s + 128 * 33;
+    for (long long it = 0; it < iters; ++it) {
+        asm volatile(
+            "red.shared.add.u32 [%0],1; red.shared.add.u32 [%1],1; red.shared.add.u32 [%2],1; red.shared.add.u32 [%3],1; "
+            "red.shared.add.u32 [%4],1; red.shared.add.u32 [%5],1; red.shared.add.u32 [%6],1; red.shared.add.u32 [%7],1;" ::
+                "r"(a0), "r"(a1), "r"(a2), "r"(a3), "r"(a4), "r"(a5), "r"(a6), "r"(a7));
+    }
+    __syncthreads();
+    if (sink && threadIdx.x == 0) sink[blockIdx.x] = a[threadIdx.x & 31];
+}
+
 // variants 3-4: the voting loop's instruction mix over a synthetic (u,v) buffer
 // (180 x 256 u16 geometry: 3 groups of 64 columns, pitch 384 B), with (4) or without (3) the atomics.
 template <bool ATOMICS>
@@ -91,7 +111,7 @@ __global__ void __launch_bounds__(1024, 1) votemix_kernel(long long iters, unsig
 }  // namespace
 
 extern "C" int hough_bench_shared_atomics(int variant, int ctas_per_sm, int threads, long long iters, double* out_rate) {
-    if (variant < 0 || variant > 4 || ctas_per_sm < 1 || threads < 32 || threads > 1024 || (threads & 31) || iters < 1 || !out_rate)
+    if (variant < 0 || variant > 5 || ctas_per_sm < 1 || threads < 32 || threads > 1024 || (threads & 31) || iters < 1 || !out_rate)
         return HOUGH_ERR_INVALID_ARG;
     int dev = 0, sms = 0;
     if (cudaGetDevice(&dev) != cudaSuccess) return HOUGH_ERR_CUDA;
@@ -99,14 +119,15 @@ extern "C" int hough_bench_shared_atomics(int variant, int ctas_per_sm, int thre
     const int grid = sms * ctas_per_sm;
     unsigned* sink = nullptr;
     if (cudaMalloc(&sink, sizeof(unsigned) * grid) != cudaSuccess) return HOUGH_ERR_NOMEM;
-    size_t smem = variant <= 2 ? 32768 : (257 * 384 + 8192);
+    size_t smem = (variant <= 2 || variant == 5) ? 32768 : (257 * 384 + 8192);
     const void* fn = nullptr;
     switch (variant) {
         case 0: fn = (const void*)&atomics_kernel<0>; break;
         case 1: fn = (const void*)&atomics_kernel<1>; break;
         case 2: fn = (const void*)&atomics_kernel<2>; break;
         case 3: fn = (const void*)&votemix_kernel<false>; break;
-        default: fn = (const void*)&votemix_kernel<true>; break;
+        case 4: fn = (const void*)&votemix_kernel<true>; break;
+        default: fn = (const void*)&atomics_peak_kernel; break;
     }
     cudaError_t e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     cudaEvent_t ev0, ev1;
@@ -123,9 +144,9 @@ extern "C" int hough_bench_shared_atomics(int variant, int ctas_per_sm, int thre
     cudaEventDestroy(ev0); cudaEventDestroy(ev1);
     cudaFree(sink);
     if (e != cudaSuccess) return HOUGH_ERR_CUDA;
-    double per_thread = variant <= 2 ? 8.0 * (double)iters : 0.0;
+    double per_thread = (variant <= 2 || variant == 5) ? 8.0 * (double)iters : 0.0;
     double total;
-    if (variant <= 2) {
+    if (variant <= 2 || variant == 5) {
         total = per_thread * (double)threads * (double)grid;
     } else {
         const int nwarps = threads / 32, n_stripes = nwarps / 3;

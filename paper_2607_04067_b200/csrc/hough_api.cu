@@ -36,6 +36,7 @@ inline int align_up(int x, int a) { return (x + a - 1) / a * a; }
 
 struct Plan {
     bool acc16 = true;
+    int cpl = 2;             // theta columns per lane in the vote phase (kernel template parameter)
     int csize = 1;
     int threads = 0;
     int smem_bytes = 0;
@@ -79,22 +80,34 @@ struct hough_ctx {
 namespace {
 
 template <bool ACC16, bool CL>
-const void* kernel_ptr() { return (const void*)&hough::hough_event_kernel<ACC16, CL>; }
+const void* kernel_ptr(int cpl) {
+    switch (cpl) {
+        case 6: return (const void*)&hough::hough_event_kernel<ACC16, CL, 6>;
+        case 4: return (const void*)&hough::hough_event_kernel<ACC16, CL, 4>;
+        default: return (const void*)&hough::hough_event_kernel<ACC16, CL, 2>;
+    }
+}
 
-const void* pick_kernel(bool acc16, bool cl) {
-    if (acc16) return cl ? kernel_ptr<true, true>() : kernel_ptr<true, false>();
-    return cl ? kernel_ptr<false, true>() : kernel_ptr<false, false>();
+const void* pick_kernel(bool acc16, bool cl, int cpl) {
+    if (acc16) return cl ? kernel_ptr<true, true>(cpl) : kernel_ptr<true, false>(cpl);
+    return cl ? kernel_ptr<false, true>(cpl) : kernel_ptr<false, false>(cpl);
 }
 
 // Lays out shared memory for cluster size C and `want_ctas` CTAs per SM.  Returns false if it does not fit.
 bool try_plan(const hough_ctx* c, bool acc16, int C, int want_ctas, Plan* out) {
     const int cols = (c->n_theta + C - 1) / C;
-    const int n_groups = (cols + 63) / 64;
+    // columns per lane: the choice that pads the fewest columns, ties to the larger (fewer broadcast loads per vote)
+    int cpl = 2, padded = 1 << 30;
+    for (int cand = 6; cand >= 2; cand -= 2) {
+        const int pc = (cols + 32 * cand - 1) / (32 * cand) * (32 * cand);
+        if (pc < padded) { padded = pc; cpl = cand; }
+    }
+    const int n_groups = padded / (32 * cpl);
     const int max_warps = want_ctas >= 2 ? 16 : 32;
     if (n_groups > max_warps) return false;
-    const int pitch_b = acc16 ? n_groups * 128 : n_groups * 256;
+    const int pitch_b = n_groups * cpl * (acc16 ? 64 : 128);
     if (pitch_b > 8192) return false;
-    const long long acc_bytes = ((long long)c->n_rho + 1) * pitch_b;   // + the trash row
+    const long long acc_bytes = (long long)c->n_rho * pitch_b + 128;   // + the 128-byte trash row
     const int wpr = (c->n_rho + 31) / 32;
     const int n_stripes = max_warps / n_groups;
     const int threads = 32 * n_groups * n_stripes;
@@ -124,6 +137,8 @@ bool try_plan(const hough_ctx* c, bool acc16, int C, int want_ctas, Plan* out) {
     kp.cols_per_cta = cols;
     kp.n_groups = n_groups;
     kp.n_stripes = n_stripes;
+    kp.vpr = pitch_b / 16;
+    kp.cand_cap = (int)chunk * 2;
     kp.pitch_b = pitch_b;
     kp.wpr = wpr;
     kp.chunk = (int)chunk;
@@ -133,6 +148,7 @@ bool try_plan(const hough_ctx* c, bool acc16, int C, int want_ctas, Plan* out) {
     kp.hb_off = (int)(region + pbm_bytes);
     kp.misc_off = kp.hb_off + (int)chunk * 8;
     out->acc16 = acc16;
+    out->cpl = cpl;
     out->csize = C;
     out->threads = threads;
     out->smem_bytes = kp.misc_off + (int)misc_bytes;
@@ -160,7 +176,7 @@ int make_plan(hough_ctx* c) {
         return fail(HOUGH_ERR_UNSUPPORTED, "a %d x %d %s accumulator does not fit the shared memory of %s",
                     c->n_theta, c->n_rho, acc16 ? "u16" : "u32",
                     c->opt_cluster ? "the requested cluster size" : "an 8-CTA cluster");
-    const void* fn = pick_kernel(best.acc16, best.csize > 1);
+    const void* fn = pick_kernel(best.acc16, best.csize > 1, best.cpl);
     CUDA_TRY(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, best.smem_bytes));
     int occ = 0;
     if (best.csize == 1) {
@@ -234,7 +250,7 @@ int launch(hough_ctx* c, const hough_io* io, cudaStream_t stream) {
     int grid = (int)std::min<long long>(want, pl.grid_max);
     grid = grid / C * C;
     if (grid < C) grid = C;
-    const void* fn = pick_kernel(pl.acc16, C > 1);
+    const void* fn = pick_kernel(pl.acc16, C > 1, pl.cpl);
     cudaLaunchConfig_t cfg{};
     cfg.gridDim = dim3((unsigned)grid);
     cfg.blockDim = dim3((unsigned)pl.threads);

@@ -4,7 +4,7 @@
 // owns one event at a time and walks a static round-robin list of events
 // (persistent grid, no scratch, re-entrant across streams).  Per event:
 //   H0/H1 stage hits -> conformal (u,v) in shared memory   PAPER.md:52-57 Eq. (1)
-//   H2/H3 vote: lane = theta column, warp-uniform hit
+//   H2/H3 vote: lane = CPL theta columns, warp-uniform hit
 //   H4    threshold + 3x3 local maximum -> peak bitmap
 //   H5    raster-order peak list
 //   H6    hit selection against the dilated peak bitmap
@@ -15,10 +15,12 @@
 // Accumulator layout in shared memory: rho-major,
 // A[k][word], so that a warp that owns 32 (or 64) adjacent theta columns hits
 // 32 distinct banks whatever the rho bins are: votes are conflict-free by
-// construction.  Local column jl = 64 g + 32 h + l  (group g, half h, lane l):
-//   u16: word g*32 + l of row k holds columns (h=0 | h=1) in its (low | high) half
-//   u32: word (2g+h)*32 + l of row k
-// Row n_rho is a trash row that swallows the out-of-range votes (never scanned).
+// construction.  Local column jl = 64 G + 32 h + l  (pair G, half h, lane l):
+//   u16: word G*32 + l of row k holds columns (h=0 | h=1) in its (low | high) half
+//   u32: word (2G+h)*32 + l of row k
+// Row n_rho is a 128-byte trash row (one word per lane) that swallows the out-of-range votes.
+// In the vote phase a warp owns a group of 32*CPL adjacent columns (CPL = 2, 4 or 6 per lane) and a
+// stripe of the hits: one broadcast LDS.64 of (u,v) feeds CPL votes per lane.
 #pragma once
 #include <cooperative_groups.h>
 #include <cuda_runtime.h>
@@ -56,8 +58,10 @@ struct KParams {
     int force_slow;
     int csize;            // CTAs per event (cluster size)
     int cols_per_cta;     // theta columns owned by one CTA
-    int n_groups;         // 64-column groups per CTA
+    int n_groups;         // groups of 32*CPL columns per CTA
     int n_stripes;        // warps per group in the vote phase
+    int vpr;              // uint4 vectors per accumulator row = pitch_b / 16
+    int cand_cap;         // capacity of the H4 candidate list (entries; lives in the hit buffer)
     int pitch_b;          // bytes per rho row of the accumulator (multiple of 128)
     int wpr;              // 32-bit words per bitmap row = ceil(n_rho / 32)
     int chunk;            // hits staged per pass
@@ -153,7 +157,7 @@ __device__ __forceinline__ unsigned cell_from(const unsigned char* acc, int pitc
 }
 
 // ---------------------------------------------------------------- the kernel
-template <bool ACC16, bool CL>
+template <bool ACC16, bool CL, int CPL>
 __global__ void __launch_bounds__(1024, 1) hough_event_kernel(const __grid_constant__ KParams p) {
     extern __shared__ __align__(128) unsigned char smem[];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -166,8 +170,8 @@ __global__ void __launch_bounds__(1024, 1) hough_event_kernel(const __grid_const
 
     unsigned char* acc = smem;                                  // accumulator region
     unsigned* pbm = (unsigned*)(smem + p.pbm_off);              // peak bitmap [cols_per_cta][wpr]
-    float2* hb = (float2*)(smem + p.hb_off);                    // staged (u,v)
-    int* misc = (int*)(smem + p.misc_off);                      // [0..32] scan scratch, [40] peak total, [41] marked count
+    float2* hb = (float2*)(smem + p.hb_off);                    // staged (u,v); H4 reuses it as the candidate list
+    int* misc = (int*)(smem + p.misc_off);                      // [0..32] scan scratch, [40] peak total, [41] marked count, [42] candidates
     const unsigned acc_s = (unsigned)__cvta_generic_to_shared(acc);
 
     const int col0 = (int)rank * p.cols_per_cta;
@@ -175,20 +179,24 @@ __global__ void __launch_bounds__(1024, 1) hough_event_kernel(const __grid_const
     if (ncols > p.cols_per_cta) ncols = p.cols_per_cta;
     if (ncols < 0) ncols = 0;
 
-    // ---- vote-phase lane constants: this lane owns local columns jl0 and jl0+32 of group g
+    // ---- vote-phase lane constants: this lane owns local columns 32*(g*CPL+q) + lane, q < CPL, of group g
     const int g = warp % p.n_groups, stripe = warp / p.n_groups;
-    const int jl0 = 64 * g + lane, jl1 = jl0 + 32;
-    const bool valid0 = jl0 < ncols, valid1 = jl1 < ncols;
-    const float c0 = valid0 ? p.cos_t[col0 + jl0] : 0.0f, s0 = valid0 ? p.sin_t[col0 + jl0] : 0.0f;
-    const float c1 = valid1 ? p.cos_t[col0 + jl1] : 0.0f, s1 = valid1 ? p.sin_t[col0 + jl1] : 0.0f;
-    const unsigned woff0 = 4u * cell_word_off<ACC16>(jl0), woff1 = 4u * cell_word_off<ACC16>(jl1);
-    const unsigned inc0 = 1u, inc1 = ACC16 ? 0x10000u : 1u;
     const unsigned pitch = (unsigned)p.pitch_b;
     const unsigned limit = (unsigned)p.n_rho * pitch;
-    // rel = (bits - MAGIC_BITS) * pitch + woff ; invalid columns are pushed out of range for good
-    const unsigned lc0 = (valid0 ? woff0 : 0x80000000u) - HOUGH_MAGIC_BITS * pitch;
-    const unsigned lc1 = (valid1 ? woff1 : 0x80000000u) - HOUGH_MAGIC_BITS * pitch;
-    const unsigned trash0 = limit + woff0, trash1 = limit + woff1;
+    const unsigned trash = limit + 4u * (unsigned)lane;        // the lane's own word of the trash row
+    float cq[CPL], sq[CPL];
+    unsigned lcq[CPL], woffq[CPL];
+    bool validq[CPL];
+#pragma unroll
+    for (int q = 0; q < CPL; ++q) {
+        const int jl = 32 * (g * CPL + q) + lane;
+        validq[q] = jl < ncols;
+        cq[q] = validq[q] ? p.cos_t[col0 + jl] : 0.0f;
+        sq[q] = validq[q] ? p.sin_t[col0 + jl] : 0.0f;
+        woffq[q] = 4u * cell_word_off<ACC16>(jl);
+        // rel = (bits - MAGIC_BITS) * pitch + woff ; invalid columns are pushed out of range for good
+        lcq[q] = (validq[q] ? woffq[q] : 0x80000000u) - HOUGH_MAGIC_BITS * pitch;
+    }
     const float rho_max = p.rho_max, inv = p.inv;
 
     const int zero_vec = (p.region_bytes + p.pbm_bytes) >> 4;   // pbm follows the region; both 16-B multiples
@@ -207,6 +215,7 @@ __global__ void __launch_bounds__(1024, 1) hough_event_kernel(const __grid_const
             uint4* z = (uint4*)smem;
             const uint4 zz = make_uint4(0, 0, 0, 0);
             for (int i = tid; i < zero_vec; i += nthreads) z[i] = zz;
+            if (tid == 0) misc[42] = 0;
         }
 
         // ---- H0-H3: stage, transform, vote (chunked)
@@ -220,49 +229,43 @@ __global__ void __launch_bounds__(1024, 1) hough_event_kernel(const __grid_const
                 tame &= (__fadd_rn(fabsf(uv.x), fabsf(uv.y)) <= p.tame_bound) ? 1 : 0;   // false for NaN/inf
             }
             const int all_tame = __shfl_sync(0xffffffffu, __syncthreads_and(tame) && !p.force_slow, 0);
-            // Every warp votes (nwarps == n_groups * n_stripes).  Hits are dealt in rounds of 4*S:
+            // Every warp votes (nwarps == n_groups * n_stripes).  Hits are dealt in rounds of 2*S:
             // the full rounds have a warp-uniform trip count, which keeps the loop in uniform
             // control flow (shared-window base in a uniform register, ATOMS [R+UR] addressing).
             const int S = p.n_stripes;
-            const int R = m / (4 * S);
+            const int R = m / (2 * S);
             if (all_tame) {
-                for (int r = 0; r < R; ++r) {
-                    float2 uv[4];
+                // out-of-range votes (rel >= limit, including every wrapped negative) land in the lane's own
+                // word of the trash row: no predicate, no branch, no conflict
+                auto vote_hit = [&](const float2 uv) {
 #pragma unroll
-                    for (int q = 0; q < 4; ++q) uv[q] = hb[(4 * r + q) * S + stripe];
-#pragma unroll
-                    for (int q = 0; q < 4; ++q) {
-                        const unsigned b0 = bin_bits(uv[q].x, uv[q].y, c0, s0, rho_max, inv);
-                        const unsigned b1 = bin_bits(uv[q].x, uv[q].y, c1, s1, rho_max, inv);
-                        // out-of-range votes (rel >= limit, including every wrapped negative) land in the
-                        // lane's own word of the trash row n_rho: no predicate, no branch, no conflict
-                        const unsigned rel0 = min(b0 * pitch + lc0, trash0);
-                        const unsigned rel1 = min(b1 * pitch + lc1, trash1);
-                        atomicAdd((unsigned*)(acc + rel0), inc0);
-                        atomicAdd((unsigned*)(acc + rel1), inc1);
+                    for (int q = 0; q < CPL; ++q) {
+                        const unsigned b = bin_bits(uv.x, uv.y, cq[q], sq[q], rho_max, inv);
+                        const unsigned rel = min(b * pitch + lcq[q], trash);
+                        atomicAdd((unsigned*)(acc + rel), (ACC16 && (q & 1)) ? 0x10000u : 1u);
                     }
+                };
+                for (int r = 0; r < R; ++r) {
+                    const float2 uv0 = hb[(2 * r) * S + stripe], uv1 = hb[(2 * r + 1) * S + stripe];
+                    vote_hit(uv0);
+                    vote_hit(uv1);
                 }
-                for (int i = 4 * R * S + stripe; i < m; i += S) {
-                    const float2 uv = hb[i];
-                    const unsigned b0 = bin_bits(uv.x, uv.y, c0, s0, rho_max, inv);
-                    const unsigned b1 = bin_bits(uv.x, uv.y, c1, s1, rho_max, inv);
-                    const unsigned rel0 = min(b0 * pitch + lc0, trash0);
-                    const unsigned rel1 = min(b1 * pitch + lc1, trash1);
-                    atomicAdd((unsigned*)(acc + rel0), inc0);
-                    atomicAdd((unsigned*)(acc + rel1), inc1);
-                }
+                for (int i = 2 * R * S + stripe; i < m; i += S) vote_hit(hb[i]);
             } else {
                 // exact slow path: literal S2 with float compares (degenerate hits: NaN, inf, r < ~0.3 mm)
                 for (int i = stripe; i < m; i += S) {
                     const float2 uv = hb[i];
-                    int k0 = bin_exact(uv.x, uv.y, c0, s0, p.rho_max, p.inv, p.n_rho);
-                    int k1 = bin_exact(uv.x, uv.y, c1, s1, p.rho_max, p.inv, p.n_rho);
-                    if (valid0 && k0 >= 0) red_shared_add(acc_s + (unsigned)k0 * pitch + woff0, inc0);
-                    if (valid1 && k1 >= 0) red_shared_add(acc_s + (unsigned)k1 * pitch + woff1, inc1);
+#pragma unroll
+                    for (int q = 0; q < CPL; ++q) {
+                        const int k = bin_exact(uv.x, uv.y, cq[q], sq[q], p.rho_max, p.inv, p.n_rho);
+                        if (validq[q] && k >= 0)
+                            red_shared_add(acc_s + (unsigned)k * pitch + woffq[q], (ACC16 && (q & 1)) ? 0x10000u : 1u);
+                    }
                 }
             }
             __syncthreads();
         }
+        if (n == 0) __syncthreads();         // no staging barrier ran: order the zeroing before the scan
         if (CL) cg::this_cluster().sync();   // (A) every CTA's columns are complete
 
         // ---- optional accumulator dump (parity / debugging; never timed)
@@ -276,11 +279,15 @@ __global__ void __launch_bounds__(1024, 1) hough_event_kernel(const __grid_const
         }
 
         // ---- H4: threshold + 3x3 local maximum -> peak bitmap (reading Q8)
+        // Pass 1 streams the accumulator as uint4 (8 u16 or 4 u32 cells) and keeps only the cells >= threshold:
+        // they go to a candidate list in the (now idle) hit buffer.  Pass 2 gives every candidate the full
+        // neighbourhood test, one candidate per thread.  A candidate that does not fit the list is tested on
+        // the spot, so the list size never decides the result.
         {
             auto cell_global = [&](int j, int k) -> unsigned {
                 if (j < 0 || j >= p.n_theta || k < 0 || k >= p.n_rho) return 0u;   // outside = 0, no theta wrap
-                int owner = j / p.cols_per_cta;
-                int jl = j - owner * p.cols_per_cta;
+                int owner = 0, jl = j;
+                if (CL) { owner = j / p.cols_per_cta; jl = j - owner * p.cols_per_cta; }
                 if (!CL || owner == (int)rank) return cell_from<ACC16>(acc, p.pitch_b, jl, k);
                 const unsigned char* racc = (const unsigned char*)cg::this_cluster().map_shared_rank((void*)acc, owner);
                 return cell_from<ACC16>(racc, p.pitch_b, jl, k);
@@ -300,19 +307,58 @@ __global__ void __launch_bounds__(1024, 1) hough_event_kernel(const __grid_const
                 }
                 if (ok) red_shared_or((unsigned)__cvta_generic_to_shared(&pbm[jl * p.wpr + (k >> 5)]), 1u << (k & 31));
             };
-            const int nwg = p.pitch_b >> 7;                 // word groups (32 words) per rho row
-            const int items = p.n_rho * nwg;
+            unsigned* cand = (unsigned*)hb;
             const unsigned thr = (unsigned)p.threshold;
-            for (int it = warp; it < items; it += nwarps) {
-                const int k = it / nwg, wg = it - k * nwg;
-                const unsigned w = *(const unsigned*)(acc + (size_t)k * p.pitch_b + 4u * (wg * 32 + lane));
+            auto candidate = [&](int jl, int k, unsigned a) {
+                if (jl >= ncols) return;                       // padding columns never hold votes; belt and braces
+                const int pos = atomicAdd(&misc[42], 1);
+                if (pos < p.cand_cap) cand[pos] = ((unsigned)k << 16) | (unsigned)jl;
+                else test_peak(jl, k, a);
+            };
+            const int vpr = p.vpr;
+            const int n_vec = p.n_rho * vpr;
+            const int step_k = nthreads / vpr, step_w = nthreads - step_k * vpr;
+            int k = tid / vpr, wv = tid - k * vpr;
+            const uint4* acc4 = (const uint4*)acc;
+            const unsigned thr2 = thr | (thr << 16);
+            for (int v = tid; v < n_vec; v += nthreads) {
+                const uint4 w = acc4[v];
+                bool any;
                 if (ACC16) {
-                    const unsigned a0 = w & 0xFFFFu, a1 = w >> 16;
-                    if (a0 >= thr) test_peak(64 * wg + lane, k, a0);
-                    if (a1 >= thr) test_peak(64 * wg + 32 + lane, k, a1);
+                    if (thr > 0xFFFFu) any = false;
+                    else {
+                        bool hi, lo;
+                        const unsigned mx = __vimax3_u16x2(__vimax3_u16x2(w.x, w.y, w.z), w.w, 0u);
+                        (void)__vibmax_u16x2(mx, thr2, &hi, &lo);
+                        any = hi || lo;
+                    }
                 } else {
-                    if (w >= thr) test_peak(32 * wg + lane, k, w);   // 32*wg + lane == 64*(wg>>1) + 32*(wg&1) + lane
+                    any = __vimax3_u32(__vimax3_u32(w.x, w.y, w.z), w.w, 0u) >= thr;
                 }
+                if (any) {
+                    const unsigned ww[4] = {w.x, w.y, w.z, w.w};
+#pragma unroll
+                    for (int i = 0; i < 4; ++i) {
+                        const int wi = 4 * wv + i;             // word index within the row
+                        if (ACC16) {
+                            const unsigned a0 = ww[i] & 0xFFFFu, a1 = ww[i] >> 16;
+                            const int jl0 = 64 * (wi >> 5) + (wi & 31);
+                            if (a0 >= thr) candidate(jl0, k, a0);
+                            if (a1 >= thr) candidate(jl0 + 32, k, a1);
+                        } else {
+                            if (ww[i] >= thr) candidate(wi, k, ww[i]);   // word (2G+h)*32 + l IS column 64G + 32h + l
+                        }
+                    }
+                }
+                wv += step_w; k += step_k;
+                if (wv >= vpr) { wv -= vpr; ++k; }
+            }
+            __syncthreads();
+            const int n_cand = min(misc[42], p.cand_cap);
+            for (int i = tid; i < n_cand; i += nthreads) {
+                const unsigned id = cand[i];
+                const int jl = (int)(id & 0xFFFFu), kk = (int)(id >> 16);
+                test_peak(jl, kk, cell_from<ACC16>(acc, p.pitch_b, jl, kk));
             }
         }
         __syncthreads();

@@ -67,7 +67,7 @@ typedef enum hough_option {
     HOUGH_OPT_CONFORMAL_SCALE = 3,  /* 1 (Eq. (1) as printed, default) or 2 (the scale Eq. (2) implies) */
     HOUGH_OPT_CLUSTER_SIZE = 4,     /* 0 = smallest of {1,2,4,8} that fits (default), else force 1,2,4,8 */
     HOUGH_OPT_CTAS_PER_SM = 5,      /* 0 = as many as fit, up to 2 (default); tuning knob */
-    HOUGH_OPT_VOTE_PATH = 6         /* 0 = fast packed-fp32 voting with the exact slow path only for
+    HOUGH_OPT_VOTE_PATH = 6         /* 0 = fast voting with packed fp32x2 arithmetic, the exact slow path only for
                                        degenerate hits (default); 1 = force the slow path (testing) */
 } hough_option;
 
@@ -171,6 +171,9 @@ const char* hough_version(void);
  *   variant 4: the voting loop's instruction mix with conflict-free atomics
  *   variant 5: the ATOMS pipe alone: eight fixed conflict-free addresses per thread, no address
  *              arithmetic in the loop (the peak the vote roofline divides by)
+ *   variant 6: variant 3 with packed fp32x2 arithmetic;  variant 7: variant 4 with packed arithmetic
+ *   variant 8: variant 7 with a 512-byte (power of two) row pitch
+ *   (variants 3, 4, 6-8 report lane-votes per second, padded lanes included)
  * Synchronises the device. */
 int hough_bench_shared_atomics(int variant, int ctas_per_sm, int threads, long long iters, double* out_rate);
 

@@ -62,6 +62,7 @@ struct hough_ctx {
     float* d_cos = nullptr;
     float* d_sin = nullptr;
     float tmax = 1.0f;
+    float tmin_nz = 1.0f;    // smallest non-zero magnitude in the trig table
     Plan plan;
     std::atomic<long long> launches{0};
     // hough_run_host staging (grow-only)
@@ -107,7 +108,14 @@ bool try_plan(const hough_ctx* c, bool acc16, int C, int want_ctas, Plan* out) {
     if (n_groups > max_warps) return false;
     const int pitch_b = n_groups * cpl * (acc16 ? 64 : 128);
     if (pitch_b > 8192) return false;
-    const long long acc_bytes = (long long)c->n_rho * pitch_b + 128;   // + the 128-byte trash row
+    const long long acc_bytes = ((long long)c->n_rho + 1) * pitch_b;   // + the trash row
+    // Padding columns carry NaN table entries; their bins are the canonical NaN (0x7FFFFFFF) and must fall
+    // beyond the accumulator after the wrapping multiply by the pitch, for every word offset of a row.
+    {
+        const unsigned nan_rel = (0x7FFFFFFFu - HOUGH_MAGIC_BITS) * (unsigned)pitch_b;
+        const unsigned long long end = (unsigned long long)(c->n_rho + 1) * (unsigned)pitch_b;
+        if ((unsigned long long)nan_rel < end || (unsigned long long)nan_rel + (unsigned)pitch_b > 0xFFFFFFFFull) return false;
+    }
     const int wpr = (c->n_rho + 31) / 32;
     const int n_stripes = max_warps / n_groups;
     const int threads = 32 * n_groups * n_stripes;
@@ -205,15 +213,19 @@ int make_plan(hough_ctx* c) {
 }
 
 int upload_table(hough_ctx* c, const float* h_cos, const float* h_sin) {
-    float tmax = 0.0f;
+    float tmax = 0.0f, tmin_nz = INFINITY;
     for (int j = 0; j < c->n_theta; ++j) {
         if (!std::isfinite(h_cos[j]) || !std::isfinite(h_sin[j]))
             return fail(HOUGH_ERR_INVALID_ARG, "trig table entry %d is not finite", j);
-        tmax = std::fmax(tmax, std::fmax(std::fabs(h_cos[j]), std::fabs(h_sin[j])));
+        const float ac = std::fabs(h_cos[j]), as = std::fabs(h_sin[j]);
+        tmax = std::fmax(tmax, std::fmax(ac, as));
+        if (ac > 0.0f) tmin_nz = std::fmin(tmin_nz, ac);
+        if (as > 0.0f) tmin_nz = std::fmin(tmin_nz, as);
     }
     CUDA_TRY(cudaMemcpy(c->d_cos, h_cos, sizeof(float) * c->n_theta, cudaMemcpyHostToDevice));
     CUDA_TRY(cudaMemcpy(c->d_sin, h_sin, sizeof(float) * c->n_theta, cudaMemcpyHostToDevice));
     c->tmax = tmax;
+    c->tmin_nz = tmin_nz;
     return HOUGH_OK;
 }
 
@@ -224,6 +236,16 @@ float tame_bound(const hough_ctx* c) {
     if (c->tmax <= 0.0f) return 3.0e38f;
     double b = 0.99 * rho_lim / (double)c->tmax;
     return b > 3.0e38 ? 3.0e38f : (float)b;
+}
+
+float ftz_min(const hough_ctx* c) {
+    // |u| >= 2^-125 / tmin_nz  =>  |u * c_j| >= 2^-125 (before rounding) for every non-zero table entry:
+    // the product is a normal number and the .ftz of the packed multiply never acts.  Never below 2^-125,
+    // so that a subnormal u or v (flushed on input) is excluded too.
+    if (!(c->tmin_nz > 0.0f) || !std::isfinite(c->tmin_nz)) return 2.3509887e-38f;   // all-zero table: nothing to flush
+    double b = std::ldexp(1.0, -125) / (double)c->tmin_nz;
+    if (b < std::ldexp(1.0, -125)) b = std::ldexp(1.0, -125);
+    return b > 3.0e38 ? 3.0e38f : (float)(b * 1.0000002);
 }
 
 int launch(hough_ctx* c, const hough_io* io, cudaStream_t stream) {
@@ -244,6 +266,7 @@ int launch(hough_ctx* c, const hough_io* io, cudaStream_t stream) {
     kp.max_peaks = c->max_peaks;
     kp.rho_max = c->rho_max; kp.inv = c->inv; kp.scale = (float)c->conformal_scale;
     kp.tame_bound = tame_bound(c);
+    kp.ftz_min = ftz_min(c);
     kp.force_slow = c->opt_vote_path == 1;
     const int C = pl.csize;
     long long want = (long long)io->n_events * C;

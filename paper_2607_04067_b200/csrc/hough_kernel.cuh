@@ -18,7 +18,7 @@
 // construction.  Local column jl = 64 G + 32 h + l  (pair G, half h, lane l):
 //   u16: word G*32 + l of row k holds columns (h=0 | h=1) in its (low | high) half
 //   u32: word (2G+h)*32 + l of row k
-// Row n_rho is a 128-byte trash row (one word per lane) that swallows the out-of-range votes.
+// Row n_rho is a trash row (one full pitch) that swallows the out-of-range votes and those of the padding columns.
 // In the vote phase a warp owns a group of 32*CPL adjacent columns (CPL = 2, 4 or 6 per lane) and a
 // stripe of the hits: one broadcast LDS.64 of (u,v) feeds CPL votes per lane.
 #pragma once
@@ -54,8 +54,9 @@ struct KParams {
     const float* sin_t;
     int n_theta, n_rho, threshold, window, max_peaks;
     float rho_max, inv, scale;
-    float tame_bound;     // a hit is "tame" iff (|u|+|v|) <= tame_bound (then |t| < 2^17 at every column)
-    int force_slow;
+    float tame_bound;     // a hit is "tame" iff (|u|+|v|) <= tame_bound (then |t| < 2^17 at every column) ...
+    float ftz_min;        // ... and u, v are each 0 or >= ftz_min in magnitude (then no product u*c, v*s is subnormal)
+    int force_slow;       // 1: literal slow path for every hit
     int csize;            // CTAs per event (cluster size)
     int cols_per_cta;     // theta columns owned by one CTA
     int n_groups;         // groups of 32*CPL columns per CTA
@@ -104,6 +105,31 @@ __device__ __forceinline__ unsigned bin_bits(float u, float v, float c, float s,
     const float rho = __fadd_rn(__fmul_rn(u, c), __fmul_rn(v, s));
     const float t = __fmul_rn(__fadd_rn(rho, rho_max), inv);
     return __float_as_uint(__fadd_rd(t, HOUGH_MAGIC_F));
+}
+
+// Two columns at once with the packed fp32x2 instructions of sm_100 (FMUL2 / FADD2): the same six
+// roundings per column as bin_bits, one instruction per PAIR of columns.  Every operation carries an
+// explicit rounding mode.  The two products are computed with .ftz: ptxas contracts a plain
+// mul.rn.f32x2 feeding an add.rn.f32x2 into FFMA2 (one rounding instead of two, seen with CUDA 12.9
+// even under --fmad=false), and it cannot do so when the flush modes differ.  The flush itself never
+// acts: the fast path only takes hits whose products with every non-zero table entry are normal
+// (KParams::ftz_min); build.py rejects any FFMA2 in the SASS.
+__device__ __forceinline__ ull pack2(float lo, float hi) {
+    ull r;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+    return r;
+}
+__device__ __forceinline__ void bin_bits2(float u, float v, ull c2, ull s2, float rho_max, float inv, unsigned& b0, unsigned& b1) {
+    const ull u2 = pack2(u, u), v2 = pack2(v, v), rm2 = pack2(rho_max, rho_max), inv2 = pack2(inv, inv);
+    const ull mg2 = pack2(HOUGH_MAGIC_F, HOUGH_MAGIC_F);
+    ull p1, p2, rho, sh, t, y;
+    asm("mul.rn.ftz.f32x2 %0, %1, %2;" : "=l"(p1) : "l"(u2), "l"(c2));
+    asm("mul.rn.ftz.f32x2 %0, %1, %2;" : "=l"(p2) : "l"(v2), "l"(s2));
+    asm("add.rn.f32x2 %0, %1, %2;" : "=l"(rho) : "l"(p1), "l"(p2));
+    asm("add.rn.f32x2 %0, %1, %2;" : "=l"(sh) : "l"(rho), "l"(rm2));
+    asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(t) : "l"(sh), "l"(inv2));
+    asm("add.rm.f32x2 %0, %1, %2;" : "=l"(y) : "l"(t), "l"(mg2));
+    asm("mov.b64 {%0, %1}, %2;" : "=r"(b0), "=r"(b1) : "l"(y));
 }
 
 // S2, scalar and literal (the slow exact path and the reference for the trick).  Returns k or -1.
@@ -183,19 +209,23 @@ __global__ void __launch_bounds__(1024, 1) hough_event_kernel(const __grid_const
     const int g = warp % p.n_groups, stripe = warp / p.n_groups;
     const unsigned pitch = (unsigned)p.pitch_b;
     const unsigned limit = (unsigned)p.n_rho * pitch;
-    const unsigned trash = limit + 4u * (unsigned)lane;        // the lane's own word of the trash row
-    float cq[CPL], sq[CPL];
-    unsigned lcq[CPL], woffq[CPL];
-    bool validq[CPL];
+    // Word of (k, column q of this lane) = k*pitch + wbase + stride*(q or q/2): one base register, the rest is an
+    // immediate of the ATOMS.  u16: columns q, q+1 share a word (low | high half), words of a lane are 128 B apart;
+    // u32: one word per column, 128 B apart.  Out-of-range bins (including every wrapped negative) are clamped to
+    // the lane's word of the trash row BEFORE the immediate is added, so they stay inside the trash row.
+    const unsigned wbase = ACC16 ? (unsigned)(g * (CPL / 2) * 128 + 4 * lane) : (unsigned)(g * CPL * 128 + 4 * lane);
+    const unsigned lc0 = wbase - HOUGH_MAGIC_BITS * pitch;     // rel = bits * pitch + lc0
+    const unsigned trash0 = limit + wbase;
+    ull c2q[CPL / 2], s2q[CPL / 2];
 #pragma unroll
-    for (int q = 0; q < CPL; ++q) {
-        const int jl = 32 * (g * CPL + q) + lane;
-        validq[q] = jl < ncols;
-        cq[q] = validq[q] ? p.cos_t[col0 + jl] : 0.0f;
-        sq[q] = validq[q] ? p.sin_t[col0 + jl] : 0.0f;
-        woffq[q] = 4u * cell_word_off<ACC16>(jl);
-        // rel = (bits - MAGIC_BITS) * pitch + woff ; invalid columns are pushed out of range for good
-        lcq[q] = (validq[q] ? woffq[q] : 0x80000000u) - HOUGH_MAGIC_BITS * pitch;
+    for (int q = 0; q < CPL; q += 2) {
+        const int j0 = 32 * (g * CPL + q) + lane, j1 = j0 + 32;
+        // a padding column gets a NaN table entry: its t is NaN at every hit and its votes end in the trash row
+        const float qnan = __uint_as_float(0x7FC00000u);
+        const float c0 = j0 < ncols ? p.cos_t[col0 + j0] : qnan, s0 = j0 < ncols ? p.sin_t[col0 + j0] : qnan;
+        const float c1 = j1 < ncols ? p.cos_t[col0 + j1] : qnan, s1 = j1 < ncols ? p.sin_t[col0 + j1] : qnan;
+        c2q[q / 2] = pack2(c0, c1);
+        s2q[q / 2] = pack2(s0, s1);
     }
     const float rho_max = p.rho_max, inv = p.inv;
 
@@ -226,7 +256,9 @@ __global__ void __launch_bounds__(1024, 1) hough_event_kernel(const __grid_const
                 float2 h = __ldg(&p.xy[beg + cbeg + i]);
                 float2 uv = conformal(h, p.scale);
                 hb[i] = uv;
-                tame &= (__fadd_rn(fabsf(uv.x), fabsf(uv.y)) <= p.tame_bound) ? 1 : 0;   // false for NaN/inf
+                const float au = fabsf(uv.x), av = fabsf(uv.y);
+                tame &= (__fadd_rn(au, av) <= p.tame_bound) ? 1 : 0;                        // false for NaN/inf
+                tame &= ((au >= p.ftz_min || au == 0.0f) && (av >= p.ftz_min || av == 0.0f)) ? 1 : 0;
             }
             const int all_tame = __shfl_sync(0xffffffffu, __syncthreads_and(tame) && !p.force_slow, 0);
             // Every warp votes (nwarps == n_groups * n_stripes).  Hits are dealt in rounds of 2*S:
@@ -239,10 +271,18 @@ __global__ void __launch_bounds__(1024, 1) hough_event_kernel(const __grid_const
                 // word of the trash row: no predicate, no branch, no conflict
                 auto vote_hit = [&](const float2 uv) {
 #pragma unroll
-                    for (int q = 0; q < CPL; ++q) {
-                        const unsigned b = bin_bits(uv.x, uv.y, cq[q], sq[q], rho_max, inv);
-                        const unsigned rel = min(b * pitch + lcq[q], trash);
-                        atomicAdd((unsigned*)(acc + rel), (ACC16 && (q & 1)) ? 0x10000u : 1u);
+                    for (int q = 0; q < CPL; q += 2) {
+                        unsigned b0, b1;
+                        bin_bits2(uv.x, uv.y, c2q[q / 2], s2q[q / 2], rho_max, inv, b0, b1);
+                        const unsigned rel0 = min(b0 * pitch + lc0, trash0);
+                        const unsigned rel1 = min(b1 * pitch + lc0, trash0);
+                        if (ACC16) {
+                            atomicAdd((unsigned*)(acc + rel0 + 128 * (q / 2)), 1u);
+                            atomicAdd((unsigned*)(acc + rel1 + 128 * (q / 2)), 0x10000u);
+                        } else {
+                            atomicAdd((unsigned*)(acc + rel0 + 128 * q), 1u);
+                            atomicAdd((unsigned*)(acc + rel1 + 128 * (q + 1)), 1u);
+                        }
                     }
                 };
                 for (int r = 0; r < R; ++r) {
@@ -255,11 +295,12 @@ __global__ void __launch_bounds__(1024, 1) hough_event_kernel(const __grid_const
                 // exact slow path: literal S2 with float compares (degenerate hits: NaN, inf, r < ~0.3 mm)
                 for (int i = stripe; i < m; i += S) {
                     const float2 uv = hb[i];
-#pragma unroll
                     for (int q = 0; q < CPL; ++q) {
-                        const int k = bin_exact(uv.x, uv.y, cq[q], sq[q], p.rho_max, p.inv, p.n_rho);
-                        if (validq[q] && k >= 0)
-                            red_shared_add(acc_s + (unsigned)k * pitch + woffq[q], (ACC16 && (q & 1)) ? 0x10000u : 1u);
+                        const int jl = 32 * (g * CPL + q) + lane;
+                        if (jl >= ncols) continue;
+                        const int k = bin_exact(uv.x, uv.y, p.cos_t[col0 + jl], p.sin_t[col0 + jl], p.rho_max, p.inv, p.n_rho);
+                        if (k >= 0)
+                            red_shared_add(acc_s + (unsigned)k * pitch + 4u * cell_word_off<ACC16>(jl), (ACC16 && (q & 1)) ? 0x10000u : 1u);
                     }
                 }
             }

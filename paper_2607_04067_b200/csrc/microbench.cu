@@ -61,13 +61,14 @@ __global__ void __launch_bounds__(1024, 1) atomics_peak_kernel(long long iters, 
     if (sink && threadIdx.x == 0) sink[blockIdx.x] = a[threadIdx.x & 31];
 }
 
-// variants 3-4: the voting loop's instruction mix over a synthetic (u,v) buffer
-// (180 x 256 u16 geometry: 3 groups of 64 columns, pitch 384 B), with (4) or without (3) the atomics.
-template <bool ATOMICS>
+// variants 3-4 and 6-8: the voting loop's instruction mix over a synthetic (u,v) buffer
+// (180 x 256 u16 geometry: 3 groups of 64 columns), with or without the atomics, scalar or packed
+// (fp32x2) arithmetic, row pitch 384 B (IMAD addressing) or 512 B (shift-add addressing).
+template <bool ATOMICS, bool PACKED, int PITCH>
 __global__ void __launch_bounds__(1024, 1) votemix_kernel(long long iters, unsigned* sink) {
     extern __shared__ __align__(128) unsigned char smem[];
-    const int N_RHO = 256, PITCH = 384, NHITS = 1024;
-    unsigned char* acc = smem;                               // 96 KB + trash row
+    const int N_RHO = 256, NHITS = 1024;
+    unsigned char* acc = smem;                               // (256 + 1 trash) rows
     float2* hb = (float2*)(smem + (N_RHO + 1) * PITCH);      // 8 KB
     for (int i = threadIdx.x; i < (N_RHO + 1) * PITCH / 4; i += blockDim.x) ((unsigned*)acc)[i] = 0;
     for (int i = threadIdx.x; i < NHITS; i += blockDim.x) {
@@ -86,14 +87,20 @@ __global__ void __launch_bounds__(1024, 1) votemix_kernel(long long iters, unsig
     const unsigned lc0 = 4u * (g * 32 + lane) - HOUGH_MAGIC_BITS * pitch, lc1 = lc0;
     const unsigned acc_s = (unsigned)__cvta_generic_to_shared(acc);
     const unsigned trash = limit + 4u * (g * 32 + lane);
+    const hough::ull C2 = hough::pack2(c0, c1), S2 = hough::pack2(s0, s1);
     unsigned chk = 0;
     if (stripe < n_stripes) {
         for (long long it = 0; it < iters; ++it) {
 #pragma unroll 4
             for (int i = stripe; i < NHITS; i += n_stripes) {
                 const float2 uv = hb[i];
-                const unsigned b0 = hough::bin_bits(uv.x, uv.y, c0, s0, rho_max, inv);
-                const unsigned b1 = hough::bin_bits(uv.x, uv.y, c1, s1, rho_max, inv);
+                unsigned b0, b1;
+                if (PACKED) {
+                    hough::bin_bits2(uv.x, uv.y, C2, S2, rho_max, inv, b0, b1);
+                } else {
+                    b0 = hough::bin_bits(uv.x, uv.y, c0, s0, rho_max, inv);
+                    b1 = hough::bin_bits(uv.x, uv.y, c1, s1, rho_max, inv);
+                }
                 const unsigned rel0 = b0 * pitch + lc0, rel1 = b1 * pitch + lc1;
                 if (ATOMICS) {
                     hough::vote_add(acc_s + min(rel0, trash), 1u);
@@ -111,7 +118,7 @@ __global__ void __launch_bounds__(1024, 1) votemix_kernel(long long iters, unsig
 }  // namespace
 
 extern "C" int hough_bench_shared_atomics(int variant, int ctas_per_sm, int threads, long long iters, double* out_rate) {
-    if (variant < 0 || variant > 5 || ctas_per_sm < 1 || threads < 32 || threads > 1024 || (threads & 31) || iters < 1 || !out_rate)
+    if (variant < 0 || variant > 8 || ctas_per_sm < 1 || threads < 32 || threads > 1024 || (threads & 31) || iters < 1 || !out_rate)
         return HOUGH_ERR_INVALID_ARG;
     int dev = 0, sms = 0;
     if (cudaGetDevice(&dev) != cudaSuccess) return HOUGH_ERR_CUDA;
@@ -119,14 +126,17 @@ extern "C" int hough_bench_shared_atomics(int variant, int ctas_per_sm, int thre
     const int grid = sms * ctas_per_sm;
     unsigned* sink = nullptr;
     if (cudaMalloc(&sink, sizeof(unsigned) * grid) != cudaSuccess) return HOUGH_ERR_NOMEM;
-    size_t smem = (variant <= 2 || variant == 5) ? 32768 : (257 * 384 + 8192);
+    size_t smem = (variant <= 2 || variant == 5) ? 32768 : (257 * (variant == 8 ? 512 : 384) + 8192);
     const void* fn = nullptr;
     switch (variant) {
         case 0: fn = (const void*)&atomics_kernel<0>; break;
         case 1: fn = (const void*)&atomics_kernel<1>; break;
         case 2: fn = (const void*)&atomics_kernel<2>; break;
-        case 3: fn = (const void*)&votemix_kernel<false>; break;
-        case 4: fn = (const void*)&votemix_kernel<true>; break;
+        case 3: fn = (const void*)&votemix_kernel<false, false, 384>; break;
+        case 4: fn = (const void*)&votemix_kernel<true, false, 384>; break;
+        case 6: fn = (const void*)&votemix_kernel<false, true, 384>; break;
+        case 7: fn = (const void*)&votemix_kernel<true, true, 384>; break;
+        case 8: fn = (const void*)&votemix_kernel<true, true, 512>; break;
         default: fn = (const void*)&atomics_peak_kernel; break;
     }
     cudaError_t e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);

@@ -207,6 +207,7 @@ def run_ours(args):
     import torch
     import paper_2607_04067_b200 as hb
     import stcf_inputs as si
+    from paper_2607_04067_b200 import shard
 
     rank, local_rank, world = dist_env()
     if not torch.cuda.is_available():
@@ -224,7 +225,8 @@ def run_ours(args):
     hb.load_library()   # raises if the CUDA library cannot be built / loaded
     w = si.config(args.config)
     n_events = args.events or min(w.n_events, 1000)
-    xy, off, _ = si.generate(w, n_events, first_event=rank * n_events)    # every rank its own events
+    first_event, _ = shard.event_range(rank, world, n_events)             # every rank its own events
+    xy, off, _ = si.generate(w, n_events, first_event=first_event)
     n_total = len(xy)
     table = si.trig_table(w.n_theta)
     h = hb.Hough(w.n_theta, w.n_rho, w.rho_max, w.threshold, w.window, max_peaks=w.max_peaks, acc_dtype=w.acc_dtype,
@@ -321,13 +323,10 @@ def run_ours(args):
 
 
     # ---- max over ranks (plumbing only)
-    agg = torch.tensor([total_ms, e2e_ms, warm_ms], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(agg, op=dist.ReduceOp.MAX)
-    total_ms, e2e_ms, warm_ms = [float(x) for x in agg.tolist()]
+    total_ms, e2e_ms, warm_ms = shard.max_over_ranks([total_ms, e2e_ms, warm_ms], device=dev)
     ms_per_step = total_ms / args.steps
-    value = world * n_events / (ms_per_step * 1e-3)
-    e2e_value = world * n_events / (e2e_ms / e2e_steps * 1e-3)
+    value = shard.job_throughput(n_events, world, ms_per_step)
+    e2e_value = shard.job_throughput(n_events, world, e2e_ms / e2e_steps)
 
     # ---- roofline of the one kernel (per launch, this rank)
     atom_rate = hb.hough_bench_shared_atomics(5, 1, 1024, 20000)          # conflict-free ATOMS/s, all SMs, measured now

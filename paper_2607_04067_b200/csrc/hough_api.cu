@@ -123,10 +123,11 @@ bool try_plan(const hough_ctx* c, bool acc16, int C, int want_ctas, Plan* out) {
     // post-extraction data that reuses the accumulator region
     long long o = 0;
     KParams kp{};
-    kp.d_off = (int)o;       o += align_up((c->n_theta + 1) * wpr * 4, 16);
-    kp.mcf_off = (int)o;     o += align_up((c->n_theta + 2) * 4, 16);
-    kp.msf_off = (int)o;     o += align_up((c->n_theta + 2) * 4, 16);
-    kp.mrow_off = (int)o;    o += align_up((c->n_theta + 2) * 4, 16);
+    kp.w8_pitch = align_up(c->n_rho + 1, 16);          // byte n_rho of a row is the always-zero clamp target
+    kp.w8_off = (int)o;      o += (long long)((c->n_theta + 7) / 8) * kp.w8_pitch;
+    kp.mcf_off = (int)o;     o += align_up((c->n_theta + 8) * 4, 16);
+    kp.msf_off = (int)o;     o += align_up((c->n_theta + 8) * 4, 16);
+    kp.colq_off = (int)o;    o += align_up(c->n_theta * 4, 16);
     kp.stash_off = (int)o;   o += (C > 1) ? align_up(HOUGH_SEL_ROUND_BLOCKS * nwarps * 4, 16) : 0;
     kp.cnt_off = (int)o;     o += (C > 1) ? align_up(HOUGH_SEL_ROUND_BLOCKS * 4, 16) : 0;
     kp.gcnt_off = (int)o;    o += (C > 1) ? align_up((HOUGH_SEL_ROUND_BLOCKS * C + 1) * 4, 16) : 0;
@@ -146,7 +147,6 @@ bool try_plan(const hough_ctx* c, bool acc16, int C, int want_ctas, Plan* out) {
     kp.n_groups = n_groups;
     kp.n_stripes = n_stripes;
     kp.vpr = pitch_b / 16;
-    kp.cand_cap = (int)chunk * 2;
     kp.pitch_b = pitch_b;
     kp.wpr = wpr;
     kp.chunk = (int)chunk;

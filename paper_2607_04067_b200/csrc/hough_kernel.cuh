@@ -62,7 +62,6 @@ struct KParams {
     int n_groups;         // groups of 32*CPL columns per CTA
     int n_stripes;        // warps per group in the vote phase
     int vpr;              // uint4 vectors per accumulator row = pitch_b / 16
-    int cand_cap;         // capacity of the H4 candidate list (entries; lives in the hit buffer)
     int pitch_b;          // bytes per rho row of the accumulator (multiple of 128)
     int wpr;              // 32-bit words per bitmap row = ceil(n_rho / 32)
     int chunk;            // hits staged per pass
@@ -72,7 +71,7 @@ struct KParams {
     int hb_off;           // hit buffer float2[chunk]
     int misc_off;         // 64 ints
     // post-extraction layout inside the accumulator region (byte offsets)
-    int d_off, mcf_off, msf_off, mrow_off, stash_off, cnt_off, gcnt_off;
+    int w8_off, w8_pitch, mcf_off, msf_off, colq_off, stash_off, cnt_off, gcnt_off;
 };
 
 // ---------------------------------------------------------------- small helpers
@@ -240,6 +239,8 @@ __global__ void __launch_bounds__(1024, 1) hough_event_kernel(const __grid_const
             continue;
         }
 
+        const bool single = n <= p.chunk;    // the whole event is staged at once: (u,v) stay in hb until selection
+
         // ---- zero accumulator + peak bitmap
         {
             uint4* z = (uint4*)smem;
@@ -348,54 +349,73 @@ __global__ void __launch_bounds__(1024, 1) hough_event_kernel(const __grid_const
                 }
                 if (ok) red_shared_or((unsigned)__cvta_generic_to_shared(&pbm[jl * p.wpr + (k >> 5)]), 1u << (k & 31));
             };
-            unsigned* cand = (unsigned*)hb;
+            // candidate list: the part of the hit buffer that holds no staged (u,v) (all of it for a multi-chunk event)
+            unsigned* cand = (unsigned*)(hb + (single ? n : 0));
+            const int cand_cap = 2 * (p.chunk - (single ? n : 0));
             const unsigned thr = (unsigned)p.threshold;
             auto candidate = [&](int jl, int k, unsigned a) {
                 if (jl >= ncols) return;                       // padding columns never hold votes; belt and braces
                 const int pos = atomicAdd(&misc[42], 1);
-                if (pos < p.cand_cap) cand[pos] = ((unsigned)k << 16) | (unsigned)jl;
+                if (pos < cand_cap) cand[pos] = ((unsigned)k << 16) | (unsigned)jl;
                 else test_peak(jl, k, a);
             };
             const int vpr = p.vpr;
             const int n_vec = p.n_rho * vpr;
-            const int step_k = nthreads / vpr, step_w = nthreads - step_k * vpr;
-            int k = tid / vpr, wv = tid - k * vpr;
             const uint4* acc4 = (const uint4*)acc;
             const unsigned thr2 = thr | (thr << 16);
-            for (int v = tid; v < n_vec; v += nthreads) {
-                const uint4 w = acc4[v];
-                bool any;
+            const bool thr_fits = !ACC16 || thr <= 0xFFFFu;     // a u16 cell can never reach a larger threshold
+            // does any cell of the vector reach the threshold?  (u16: packed 3-input max, then one packed compare)
+            auto vec_any = [&](const uint4& w) -> bool {
                 if (ACC16) {
-                    if (thr > 0xFFFFu) any = false;
-                    else {
-                        bool hi, lo;
-                        const unsigned mx = __vimax3_u16x2(__vimax3_u16x2(w.x, w.y, w.z), w.w, 0u);
-                        (void)__vibmax_u16x2(mx, thr2, &hi, &lo);
-                        any = hi || lo;
-                    }
-                } else {
-                    any = __vimax3_u32(__vimax3_u32(w.x, w.y, w.z), w.w, 0u) >= thr;
+                    bool hi, lo;
+                    const unsigned mx = __vimax3_u16x2(__vimax3_u16x2(w.x, w.y, w.z), w.w, 0u);
+                    (void)__vibmax_u16x2(mx, thr2, &hi, &lo);   // hi/lo: that half of mx is >= thr
+                    return (hi || lo) && thr_fits;
                 }
-                if (any) {
-                    const unsigned ww[4] = {w.x, w.y, w.z, w.w};
+                return __vimax3_u32(__vimax3_u32(w.x, w.y, w.z), w.w, 0u) >= thr;
+            };
+            auto scan_vec = [&](int v, const uint4& w) {       // rare at a sensible threshold: the index arithmetic lives here
+                if (!vec_any(w)) return;
+                const int k = v / vpr, wv = v - k * vpr;
+                const unsigned ww[4] = {w.x, w.y, w.z, w.w};
 #pragma unroll
-                    for (int i = 0; i < 4; ++i) {
-                        const int wi = 4 * wv + i;             // word index within the row
-                        if (ACC16) {
-                            const unsigned a0 = ww[i] & 0xFFFFu, a1 = ww[i] >> 16;
-                            const int jl0 = 64 * (wi >> 5) + (wi & 31);
-                            if (a0 >= thr) candidate(jl0, k, a0);
-                            if (a1 >= thr) candidate(jl0 + 32, k, a1);
-                        } else {
-                            if (ww[i] >= thr) candidate(wi, k, ww[i]);   // word (2G+h)*32 + l IS column 64G + 32h + l
-                        }
+                for (int i = 0; i < 4; ++i) {
+                    const int wi = 4 * wv + i;                 // word index within the row
+                    if (ACC16) {
+                        const unsigned a0 = ww[i] & 0xFFFFu, a1 = ww[i] >> 16;
+                        const int jl0 = 64 * (wi >> 5) + (wi & 31);
+                        if (a0 >= thr) candidate(jl0, k, a0);
+                        if (a1 >= thr) candidate(jl0 + 32, k, a1);
+                    } else {
+                        if (ww[i] >= thr) candidate(wi, k, ww[i]);   // word (2G+h)*32 + l IS column 64G + 32h + l
                     }
                 }
-                wv += step_w; k += step_k;
-                if (wv >= vpr) { wv -= vpr; ++k; }
+            };
+            int v = tid;
+            for (; v + 3 * nthreads < n_vec; v += 4 * nthreads) {   // four vectors per trip, one test
+                const uint4 w0 = acc4[v], w1 = acc4[v + nthreads], w2 = acc4[v + 2 * nthreads], w3 = acc4[v + 3 * nthreads];
+                bool any4;                                         // max over the 16 words: eight 3-input max, one compare
+                if (ACC16) {
+                    unsigned m = __vimax3_u16x2(w0.x, w0.y, w0.z);
+                    m = __vimax3_u16x2(m, w0.w, w1.x); m = __vimax3_u16x2(m, w1.y, w1.z); m = __vimax3_u16x2(m, w1.w, w2.x);
+                    m = __vimax3_u16x2(m, w2.y, w2.z); m = __vimax3_u16x2(m, w2.w, w3.x); m = __vimax3_u16x2(m, w3.y, w3.z);
+                    m = __vimax3_u16x2(m, w3.w, 0u);
+                    bool hi, lo;
+                    (void)__vibmax_u16x2(m, thr2, &hi, &lo);
+                    any4 = (hi || lo) && thr_fits;
+                } else {
+                    unsigned m = __vimax3_u32(w0.x, w0.y, w0.z);
+                    m = __vimax3_u32(m, w0.w, w1.x); m = __vimax3_u32(m, w1.y, w1.z); m = __vimax3_u32(m, w1.w, w2.x);
+                    m = __vimax3_u32(m, w2.y, w2.z); m = __vimax3_u32(m, w2.w, w3.x); m = __vimax3_u32(m, w3.y, w3.z);
+                    any4 = __vimax3_u32(m, w3.w, 0u) >= thr;
+                }
+                if (any4) {
+                    scan_vec(v, w0); scan_vec(v + nthreads, w1); scan_vec(v + 2 * nthreads, w2); scan_vec(v + 3 * nthreads, w3);
+                }
             }
+            for (; v < n_vec; v += nthreads) scan_vec(v, acc4[v]);
             __syncthreads();
-            const int n_cand = min(misc[42], p.cand_cap);
+            const int n_cand = min(misc[42], cand_cap);
             for (int i = tid; i < n_cand; i += nthreads) {
                 const unsigned id = cand[i];
                 const int jl = (int)(id & 0xFFFFu), kk = (int)(id >> 16);
@@ -447,37 +467,34 @@ __global__ void __launch_bounds__(1024, 1) hough_event_kernel(const __grid_const
             __syncthreads();
         }
 
-        // ---- H6 set-up: dilated bitmap D[n_theta+1][wpr] (union of the stored peaks' windows; row n_theta = zero dummy)
-        unsigned* D = (unsigned*)(acc + p.d_off);
+        // ---- H6 set-up.  Marked columns = theta columns inside some stored peak's window; they get consecutive
+        // indices q.  W8[q/8][k] is a byte whose bit (q%8) says "bin k of marked column q lies in a stored peak's
+        // window" (= the union of the windows, S5).  Byte n_rho of a row stays 0: the clamp target of invalid bins.
+        unsigned char* W8 = acc + p.w8_off;
         float* mcf = (float*)(acc + p.mcf_off);
         float* msf = (float*)(acc + p.msf_off);
-        int* mrow = (int*)(acc + p.mrow_off);
-        const int d_words = (p.n_theta + 1) * p.wpr;
-        for (int i = tid; i < d_words; i += nthreads) D[i] = 0u;
-        if (tid == 0) misc[41] = 0;
+        int* colq = (int*)(acc + p.colq_off);
+        {
+            long long cols_ub = (long long)n_stored * (2LL * p.window + 1);
+            if (cols_ub > p.n_theta) cols_ub = p.n_theta;
+            const int w8_vec = (int)((cols_ub + 7) >> 3) * (p.w8_pitch >> 4);
+            uint4* z = (uint4*)W8;
+            const uint4 zz = make_uint4(0, 0, 0, 0);
+            for (int i = tid; i < w8_vec; i += nthreads) z[i] = zz;
+            for (int j = tid; j < p.n_theta; j += nthreads) colq[j] = 0;
+            if (tid == 0) misc[41] = 0;
+        }
         __syncthreads();
         for (int q = tid; q < n_stored; q += nthreads) {
             const hough_peak pk = p.peaks[(size_t)e * p.max_peaks + q];
             const int jlo = max(0, (int)pk.theta_bin - p.window), jhi = min(p.n_theta - 1, (int)pk.theta_bin + p.window);
-            const int klo = max(0, (int)pk.rho_bin - p.window), khi = min(p.n_rho - 1, (int)pk.rho_bin + p.window);
-            for (int j = jlo; j <= jhi; ++j) {
-                for (int wd = klo >> 5; wd <= khi >> 5; ++wd) {
-                    const int a = max(klo, wd << 5) & 31, b = min(khi, (wd << 5) + 31) & 31;
-                    const unsigned mask = (0xFFFFFFFFu >> (31 - b)) & (0xFFFFFFFFu << a);
-                    red_shared_or((unsigned)__cvta_generic_to_shared(&D[j * p.wpr + wd]), mask);
-                }
-            }
+            for (int j = jlo; j <= jhi; ++j) colq[j] = 1;
         }
         __syncthreads();
-        // marked columns: those with any bit set (order irrelevant for the OR below)
+        // number the marked columns (order irrelevant for the OR of S5)
         for (int jb = 0; jb < p.n_theta; jb += nthreads) {
             const int j = jb + tid;
-            bool any = false;
-            if (j < p.n_theta) {
-                unsigned o = 0;
-                for (int wd = 0; wd < p.wpr; ++wd) o |= D[j * p.wpr + wd];
-                any = o != 0u;
-            }
+            const bool any = j < p.n_theta && colq[j] != 0;
             const unsigned bal = __ballot_sync(0xffffffffu, any);
             int wbase = 0;
             if (lane == 0 && bal) wbase = atomicAdd(&misc[41], __popc(bal));
@@ -486,30 +503,51 @@ __global__ void __launch_bounds__(1024, 1) hough_event_kernel(const __grid_const
                 const int q = wbase + __popc(bal & ((1u << lane) - 1u));
                 mcf[q] = p.cos_t[j];
                 msf[q] = p.sin_t[j];
-                mrow[q] = j * p.wpr;
+                colq[j] = q;
             }
         }
         __syncthreads();
-        int n_marked = misc[41];
-        if (n_marked & 1) {   // pad to a pair with a column that can never keep (zero dummy row)
-            if (tid == 0) { mcf[n_marked] = 0.0f; msf[n_marked] = 0.0f; mrow[n_marked] = p.n_theta * p.wpr; }
-            ++n_marked;
+        const int n_marked = misc[41];
+        const int n_g8 = (n_marked + 7) >> 3;
+        if (tid < 8 * n_g8 - n_marked) {   // pad the last group with columns whose bits are never set
+            mcf[n_marked + tid] = 0.0f;
+            msf[n_marked + tid] = 0.0f;
+        }
+        for (int q = tid; q < n_stored; q += nthreads) {
+            const hough_peak pk = p.peaks[(size_t)e * p.max_peaks + q];
+            const int jlo = max(0, (int)pk.theta_bin - p.window), jhi = min(p.n_theta - 1, (int)pk.theta_bin + p.window);
+            const int klo = max(0, (int)pk.rho_bin - p.window), khi = min(p.n_rho - 1, (int)pk.rho_bin + p.window);
+            for (int j = jlo; j <= jhi; ++j) {
+                const int cq = colq[j];
+                const unsigned bit4 = (1u << (cq & 7)) * 0x01010101u;
+                const unsigned row_s = (unsigned)__cvta_generic_to_shared(W8 + (cq >> 3) * p.w8_pitch);
+                for (int wd = klo >> 2; wd <= khi >> 2; ++wd) {
+                    const int a = max(klo, wd << 2) & 3, b = min(khi, (wd << 2) + 3) & 3;
+                    const unsigned bytes = (0xFFFFFFFFu >> (8 * (3 - b))) & (0xFFFFFFFFu << (8 * a));
+                    red_shared_or(row_s + 4u * wd, bit4 & bytes);
+                }
+            }
         }
         __syncthreads();
 
-        // keep test of one hit: OR over marked columns of D[j][bin(i,j)]  (== S5)
+        // keep test of one hit: OR over the marked columns q of bit q of W8[.][bin(i, column q)]  (== S5)
+        const unsigned n_rho_u = (unsigned)p.n_rho;
         auto keep_test = [&](float2 uv, bool valid) -> bool {
-            bool kp = false;
-            for (int mq = 0; mq < n_marked; mq += 2) {
-                const float2 mc = *(const float2*)(mcf + mq), ms = *(const float2*)(msf + mq);
-                const int2 rows = *(const int2*)(mrow + mq);
-                const unsigned k0 = bin_bits(uv.x, uv.y, mc.x, ms.x, rho_max, inv) - HOUGH_MAGIC_BITS;
-                const unsigned k1 = bin_bits(uv.x, uv.y, mc.y, ms.y, rho_max, inv) - HOUGH_MAGIC_BITS;
-                if (k0 < (unsigned)p.n_rho) kp = kp || ((D[rows.x + (k0 >> 5)] >> (k0 & 31)) & 1u);
-                if (k1 < (unsigned)p.n_rho) kp = kp || ((D[rows.y + (k1 >> 5)] >> (k1 & 31)) & 1u);
-                if ((mq & 6) == 6 && __all_sync(0xffffffffu, kp || !valid)) break;
+            unsigned hitbits = 0;
+            for (int g8 = 0; g8 < n_g8; ++g8) {
+                const float4 ca = *(const float4*)(mcf + 8 * g8), cb = *(const float4*)(mcf + 8 * g8 + 4);
+                const float4 sa = *(const float4*)(msf + 8 * g8), sb = *(const float4*)(msf + 8 * g8 + 4);
+                const unsigned char* row = W8 + g8 * p.w8_pitch;
+                const float cc[8] = {ca.x, ca.y, ca.z, ca.w, cb.x, cb.y, cb.z, cb.w};
+                const float ss[8] = {sa.x, sa.y, sa.z, sa.w, sb.x, sb.y, sb.z, sb.w};
+#pragma unroll
+                for (int i = 0; i < 8; ++i) {
+                    const unsigned k = min(bin_bits(uv.x, uv.y, cc[i], ss[i], rho_max, inv) - HOUGH_MAGIC_BITS, n_rho_u);
+                    hitbits |= (unsigned)row[k] & (1u << i);
+                }
+                if (__all_sync(0xffffffffu, hitbits != 0u || !valid)) break;
             }
-            return kp && valid;
+            return hitbits != 0u && valid;
         };
 
         // ---- H6 + H7
@@ -518,15 +556,15 @@ __global__ void __launch_bounds__(1024, 1) hough_event_kernel(const __grid_const
             for (int b0i = 0; b0i < n; b0i += nthreads) {
                 const int i = b0i + tid;
                 const bool valid = i < n;
-                float2 h = make_float2(1.0f, 0.0f);
-                if (valid) h = __ldg(&p.xy[beg + i]);
-                const bool kp = keep_test(conformal(h, p.scale), valid);
+                float2 uv = make_float2(0.0f, 0.0f);
+                if (valid) uv = single ? hb[i] : conformal(__ldg(&p.xy[beg + i]), p.scale);
+                const bool kp = keep_test(uv, valid);
                 int blk_total;
                 const int ppos = block_exscan(kp ? 1 : 0, misc, blk_total);
                 if (valid) {
                     p.keep[beg + i] = kp ? 1 : 0;
                     if (kp) {
-                        if (p.kept_xy) p.kept_xy[beg + kept_base + ppos] = h;
+                        if (p.kept_xy) p.kept_xy[beg + kept_base + ppos] = __ldg(&p.xy[beg + i]);
                         if (p.kept_idx) p.kept_idx[beg + kept_base + ppos] = i;
                     }
                 }
@@ -547,9 +585,9 @@ __global__ void __launch_bounds__(1024, 1) hough_event_kernel(const __grid_const
                 for (int bl = 0; rb + bl * C + (int)rank < rb + rnb; ++bl) {
                     const int i = (rb + bl * C + (int)rank) * nthreads + tid;
                     const bool valid = i < n;
-                    float2 h = make_float2(1.0f, 0.0f);
-                    if (valid) h = __ldg(&p.xy[beg + i]);
-                    const bool kp = keep_test(conformal(h, p.scale), valid);
+                    float2 uv = make_float2(0.0f, 0.0f);
+                    if (valid) uv = single ? hb[i] : conformal(__ldg(&p.xy[beg + i]), p.scale);
+                    const bool kp = keep_test(uv, valid);
                     const unsigned bal = __ballot_sync(0xffffffffu, kp);
                     if (lane == 0) stash[bl * nwarps + warp] = bal;
                     if (valid) p.keep[beg + i] = kp ? 1 : 0;

@@ -68,7 +68,9 @@ typedef enum hough_option {
     HOUGH_OPT_CLUSTER_SIZE = 4,     /* 0 = smallest of {1,2,4,8} that fits (default), else force 1,2,4,8 */
     HOUGH_OPT_CTAS_PER_SM = 5,      /* 0 = as many as fit, up to 2 (default); tuning knob */
     HOUGH_OPT_VOTE_PATH = 6         /* 0 = fast voting with packed fp32x2 arithmetic, the exact slow path only for
-                                       degenerate hits (default); 1 = force the slow path (testing) */
+                                       degenerate hits (default); 1 = force the slow path (testing);
+                                       2, 3 = timing diagnostics whose OUTPUTS ARE UNDEFINED: 2 skips the voting loops,
+                                       3 skips everything after voting (bench.py --vote-path) */
 } hough_option;
 
 enum { HOUGH_ACC_AUTO = 0, HOUGH_ACC_U16 = 1, HOUGH_ACC_U32 = 2 };

@@ -268,9 +268,11 @@ int launch(hough_ctx* c, const hough_io* io, cudaStream_t stream) {
     kp.tame_bound = tame_bound(c);
     kp.ftz_min = ftz_min(c);
     kp.force_slow = c->opt_vote_path == 1;
+    kp.diag = c->opt_vote_path >= 2 ? c->opt_vote_path : 0;
     const int C = pl.csize;
     long long want = (long long)io->n_events * C;
-    int grid = (int)std::min<long long>(want, pl.grid_max);
+    const long long cap = getenv("HOUGH_PERSISTENT") ? (long long)pl.grid_max : 0x7FFFFFF0LL;
+    int grid = (int)std::min<long long>(want, cap);
     grid = grid / C * C;
     if (grid < C) grid = C;
     const void* fn = pick_kernel(pl.acc16, C > 1, pl.cpl);
@@ -359,7 +361,7 @@ int hough_set_option(hough_ctx* c, int key, long long value) {
             if (value < 0 || value > 2) return fail(HOUGH_ERR_INVALID_ARG, "ctas_per_sm must be 0,1,2");
             c->opt_ctas_per_sm = (int)value; break;
         case HOUGH_OPT_VOTE_PATH:
-            if (value != 0 && value != 1) return fail(HOUGH_ERR_INVALID_ARG, "vote path must be 0 or 1");
+            if (value < 0 || value > 3) return fail(HOUGH_ERR_INVALID_ARG, "vote path must be 0..3");
             c->opt_vote_path = (int)value; return HOUGH_OK;
         default:
             return fail(HOUGH_ERR_INVALID_ARG, "unknown option %d", key);

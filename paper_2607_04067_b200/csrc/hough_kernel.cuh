@@ -57,6 +57,7 @@ struct KParams {
     float tame_bound;     // a hit is "tame" iff (|u|+|v|) <= tame_bound (then |t| < 2^17 at every column) ...
     float ftz_min;        // ... and u, v are each 0 or >= ftz_min in magnitude (then no product u*c, v*s is subnormal)
     int force_slow;       // 1: literal slow path for every hit
+    int diag;             // timing diagnostics (outputs undefined): 2 = skip the vote loops, 3 = skip everything after voting
     int csize;            // CTAs per event (cluster size)
     int cols_per_cta;     // theta columns owned by one CTA
     int n_groups;         // groups of 32*CPL columns per CTA
@@ -267,7 +268,8 @@ __global__ void __launch_bounds__(1024, 1) hough_event_kernel(const __grid_const
             // control flow (shared-window base in a uniform register, ATOMS [R+UR] addressing).
             const int S = p.n_stripes;
             const int R = m / (2 * S);
-            if (all_tame) {
+            if (p.diag == 2) {
+            } else if (all_tame) {
                 // out-of-range votes (rel >= limit, including every wrapped negative) land in the lane's own
                 // word of the trash row: no predicate, no branch, no conflict
                 auto vote_hit = [&](const float2 uv) {
@@ -310,6 +312,8 @@ __global__ void __launch_bounds__(1024, 1) hough_event_kernel(const __grid_const
         if (n == 0) __syncthreads();         // no staging barrier ran: order the zeroing before the scan
         if (CL) cg::this_cluster().sync();   // (A) every CTA's columns are complete
 
+        if (p.diag == 3) { __syncthreads(); continue; }
+
         // ---- optional accumulator dump (parity / debugging; never timed)
         if (p.accum_dump) {
             unsigned* dst = p.accum_dump + ((size_t)e * p.n_theta + col0) * p.n_rho;
@@ -326,27 +330,38 @@ __global__ void __launch_bounds__(1024, 1) hough_event_kernel(const __grid_const
         // neighbourhood test, one candidate per thread.  A candidate that does not fit the list is tested on
         // the spot, so the list size never decides the result.
         {
-            auto cell_global = [&](int j, int k) -> unsigned {
-                if (j < 0 || j >= p.n_theta || k < 0 || k >= p.n_rho) return 0u;   // outside = 0, no theta wrap
-                int owner = 0, jl = j;
-                if (CL) { owner = j / p.cols_per_cta; jl = j - owner * p.cols_per_cta; }
-                if (!CL || owner == (int)rank) return cell_from<ACC16>(acc, p.pitch_b, jl, k);
-                const unsigned char* racc = (const unsigned char*)cg::this_cluster().map_shared_rank((void*)acc, owner);
-                return cell_from<ACC16>(racc, p.pitch_b, jl, k);
-            };
+            // 3x3 test of one cell (reading Q8).  Branch-free: every neighbour is loaded from a clamped (always
+            // valid) address and replaced by 0 when it lies outside the array, so the eight loads are independent.
             auto test_peak = [&](int jl, int k, unsigned a) {
                 const int j = col0 + jl;
-                bool ok = true;
+                const int km = max(k - 1, 0), kp1 = min(k + 1, p.n_rho - 1);
+                const bool vkm = k > 0, vkp = k + 1 < p.n_rho;
+                unsigned nb[3][3];
 #pragma unroll
                 for (int dj = -1; dj <= 1; ++dj) {
-#pragma unroll
-                    for (int dk = -1; dk <= 1; ++dk) {
-                        if (dj == 0 && dk == 0) continue;
-                        const unsigned nb = cell_global(j + dj, k + dk);
-                        const bool precedes = (dj < 0) || (dj == 0 && dk < 0);
-                        ok = ok && (precedes ? (a > nb) : (a >= nb));
+                    const int jj = j + dj;
+                    const bool vj = jj >= 0 && jj < p.n_theta;
+                    const int jc = min(max(jj, 0), p.n_theta - 1);
+                    const unsigned char* base = acc;
+                    int jcl = jc;
+                    if (CL) {
+                        const int owner = jc / p.cols_per_cta;
+                        jcl = jc - owner * p.cols_per_cta;
+                        if (owner != (int)rank) base = (const unsigned char*)cg::this_cluster().map_shared_rank((void*)acc, owner);
                     }
+                    const unsigned char* colp = base + 4u * cell_word_off<ACC16>(jcl);
+                    const int sh = ACC16 ? 16 * ((jcl >> 5) & 1) : 0;
+                    const unsigned w0 = *(const unsigned*)(colp + (size_t)km * p.pitch_b);
+                    const unsigned w1 = *(const unsigned*)(colp + (size_t)k * p.pitch_b);
+                    const unsigned w2 = *(const unsigned*)(colp + (size_t)kp1 * p.pitch_b);
+                    const unsigned msk = ACC16 ? 0xFFFFu : 0xFFFFFFFFu;
+                    nb[dj + 1][0] = (vj && vkm) ? ((w0 >> sh) & msk) : 0u;
+                    nb[dj + 1][1] = vj ? ((w1 >> sh) & msk) : 0u;
+                    nb[dj + 1][2] = (vj && vkp) ? ((w2 >> sh) & msk) : 0u;
                 }
+                // strictly greater than the neighbours that precede in raster order, >= those that follow
+                const bool ok = a > nb[0][0] && a > nb[0][1] && a > nb[0][2] && a > nb[1][0] &&
+                                a >= nb[1][2] && a >= nb[2][0] && a >= nb[2][1] && a >= nb[2][2];
                 if (ok) red_shared_or((unsigned)__cvta_generic_to_shared(&pbm[jl * p.wpr + (k >> 5)]), 1u << (k & 31));
             };
             // candidate list: the part of the hit buffer that holds no staged (u,v) (all of it for a multi-chunk event)

@@ -146,6 +146,12 @@ bool try_plan(const hough_ctx* c, bool acc16, int C, int want_ctas, Plan* out) {
     kp.cols_per_cta = cols;
     kp.n_groups = n_groups;
     kp.n_stripes = n_stripes;
+    kp.rcp_groups = 65536u / (unsigned)n_groups + 1u;
+    kp.rcp_2s = (1u << 20) / (unsigned)(2 * n_stripes) + 1u;
+    for (unsigned w = 0; w < 32; ++w)
+        if (((w * kp.rcp_groups) >> 16) != w / (unsigned)n_groups) return false;
+    for (unsigned m = 0; m <= (unsigned)chunk; ++m)
+        if (((m * kp.rcp_2s) >> 20) != m / (unsigned)(2 * n_stripes)) return false;
     kp.vpr = pitch_b / 16;
     kp.pitch_b = pitch_b;
     kp.wpr = wpr;

@@ -62,6 +62,8 @@ struct KParams {
     int cols_per_cta;     // theta columns owned by one CTA
     int n_groups;         // groups of 32*CPL columns per CTA
     int n_stripes;        // warps per group in the vote phase
+    unsigned rcp_groups;  // (warp * rcp_groups) >> 16 == warp / n_groups for warp < 32 (checked by the planner)
+    unsigned rcp_2s;      // (m * rcp_2s) >> 20 == m / (2 * n_stripes) for m <= chunk (checked by the planner)
     int vpr;              // uint4 vectors per accumulator row = pitch_b / 16
     int pitch_b;          // bytes per rho row of the accumulator (multiple of 128)
     int wpr;              // 32-bit words per bitmap row = ceil(n_rho / 32)
@@ -192,7 +194,11 @@ __global__ void __launch_bounds__(1024, 1) hough_event_kernel(const __grid_const
     unsigned rank = 0;
     if (CL) rank = cg::this_cluster().block_rank();
     const int C = p.csize;
-    const int cluster_id = blockIdx.x / C, n_clusters = gridDim.x / C;
+    int cluster_id = blockIdx.x, n_clusters = gridDim.x;
+    if (CL) {   // the hardware's own cluster index: no division by the run-time cluster size
+        asm("mov.u32 %0, %%clusterid.x;" : "=r"(cluster_id));
+        asm("mov.u32 %0, %%nclusterid.x;" : "=r"(n_clusters));
+    }
 
     unsigned char* acc = smem;                                  // accumulator region
     unsigned* pbm = (unsigned*)(smem + p.pbm_off);              // peak bitmap [cols_per_cta][wpr]
@@ -206,7 +212,7 @@ __global__ void __launch_bounds__(1024, 1) hough_event_kernel(const __grid_const
     if (ncols < 0) ncols = 0;
 
     // ---- vote-phase lane constants: this lane owns local columns 32*(g*CPL+q) + lane, q < CPL, of group g
-    const int g = warp % p.n_groups, stripe = warp / p.n_groups;
+    const int stripe = (int)(((unsigned)warp * p.rcp_groups) >> 16), g = warp - stripe * p.n_groups;
     const unsigned pitch = (unsigned)p.pitch_b;
     const unsigned limit = (unsigned)p.n_rho * pitch;
     // Word of (k, column q of this lane) = k*pitch + wbase + stride*(q or q/2): one base register, the rest is an
@@ -242,6 +248,11 @@ __global__ void __launch_bounds__(1024, 1) hough_event_kernel(const __grid_const
 
         const bool single = n <= p.chunk;    // the whole event is staged at once: (u,v) stay in hb until selection
 
+        // the first two hits of this thread are requested before the zeroing stores, which then overlap the latency
+        float2 pre0 = make_float2(1.0f, 0.0f), pre1 = pre0;
+        if (tid < n) pre0 = __ldg(&p.xy[beg + tid]);
+        if (tid + nthreads < n) pre1 = __ldg(&p.xy[beg + tid + nthreads]);
+
         // ---- zero accumulator + peak bitmap
         {
             uint4* z = (uint4*)smem;
@@ -255,7 +266,10 @@ __global__ void __launch_bounds__(1024, 1) hough_event_kernel(const __grid_const
             const int m = min(p.chunk, n - cbeg);
             int tame = 1;
             for (int i = tid; i < m; i += nthreads) {
-                float2 h = __ldg(&p.xy[beg + cbeg + i]);
+                float2 h;
+                if (cbeg == 0 && i == tid) h = pre0;
+                else if (cbeg == 0 && i == tid + nthreads) h = pre1;
+                else h = __ldg(&p.xy[beg + cbeg + i]);
                 float2 uv = conformal(h, p.scale);
                 hb[i] = uv;
                 const float au = fabsf(uv.x), av = fabsf(uv.y);
@@ -267,7 +281,7 @@ __global__ void __launch_bounds__(1024, 1) hough_event_kernel(const __grid_const
             // the full rounds have a warp-uniform trip count, which keeps the loop in uniform
             // control flow (shared-window base in a uniform register, ATOMS [R+UR] addressing).
             const int S = p.n_stripes;
-            const int R = m / (2 * S);
+            const int R = (int)(((unsigned)m * p.rcp_2s) >> 20);   // m / (2 * S)
             if (p.diag == 2) {
             } else if (all_tame) {
                 // out-of-range votes (rel >= limit, including every wrapped negative) land in the lane's own
@@ -325,10 +339,6 @@ __global__ void __launch_bounds__(1024, 1) hough_event_kernel(const __grid_const
         }
 
         // ---- H4: threshold + 3x3 local maximum -> peak bitmap (reading Q8)
-        // Pass 1 streams the accumulator as uint4 (8 u16 or 4 u32 cells) and keeps only the cells >= threshold:
-        // they go to a candidate list in the (now idle) hit buffer.  Pass 2 gives every candidate the full
-        // neighbourhood test, one candidate per thread.  A candidate that does not fit the list is tested on
-        // the spot, so the list size never decides the result.
         {
             // 3x3 test of one cell (reading Q8).  Branch-free: every neighbour is loaded from a clamped (always
             // valid) address and replaced by 0 when it lies outside the array, so the eight loads are independent.
@@ -364,17 +374,24 @@ __global__ void __launch_bounds__(1024, 1) hough_event_kernel(const __grid_const
                                 a >= nb[1][2] && a >= nb[2][0] && a >= nb[2][1] && a >= nb[2][2];
                 if (ok) red_shared_or((unsigned)__cvta_generic_to_shared(&pbm[jl * p.wpr + (k >> 5)]), 1u << (k & 31));
             };
-            // candidate list: the part of the hit buffer that holds no staged (u,v) (all of it for a multi-chunk event)
-            unsigned* cand = (unsigned*)(hb + (single ? n : 0));
-            const int cand_cap = 2 * (p.chunk - (single ? n : 0));
+            // Pass 1 streams the accumulator as uint4 and lists the VECTORS that hold a cell >= threshold (the list
+            // lives in the part of the hit buffer without staged (u,v)); pass 2 gives every cell of a listed vector
+            // its own thread.  A vector that does not fit the list is handled on the spot, so the list size never
+            // decides the result.
+            unsigned* vlist = (unsigned*)(hb + (single ? n : 0));
+            const int vcap = 2 * (p.chunk - (single ? n : 0));
             const unsigned thr = (unsigned)p.threshold;
-            auto candidate = [&](int jl, int k, unsigned a) {
-                if (jl >= ncols) return;                       // padding columns never hold votes; belt and braces
-                const int pos = atomicAdd(&misc[42], 1);
-                if (pos < cand_cap) cand[pos] = ((unsigned)k << 16) | (unsigned)jl;
-                else test_peak(jl, k, a);
-            };
             const int vpr = p.vpr;
+            constexpr int CELLS = ACC16 ? 8 : 4;               // cells per uint4
+            auto test_cell = [&](int v, int c) {
+                const int k = v / vpr, wv = v - k * vpr;
+                const int wi = 4 * wv + (ACC16 ? (c >> 1) : c);  // word index within the row
+                const unsigned word = *(const unsigned*)(acc + (size_t)k * p.pitch_b + 4u * wi);
+                // u16: word G*32 + l holds columns 64G + l (low half) and 64G + 32 + l (high half); u32: word index IS the column
+                const int jl = ACC16 ? 64 * (wi >> 5) + (wi & 31) + 32 * (c & 1) : wi;
+                const unsigned a = ACC16 ? ((word >> (16 * (c & 1))) & 0xFFFFu) : word;
+                if (a >= thr && jl < ncols) test_peak(jl, k, a);   // padding columns never hold votes; belt and braces
+            };
             const int n_vec = p.n_rho * vpr;
             const uint4* acc4 = (const uint4*)acc;
             const unsigned thr2 = thr | (thr << 16);
@@ -389,22 +406,12 @@ __global__ void __launch_bounds__(1024, 1) hough_event_kernel(const __grid_const
                 }
                 return __vimax3_u32(__vimax3_u32(w.x, w.y, w.z), w.w, 0u) >= thr;
             };
-            auto scan_vec = [&](int v, const uint4& w) {       // rare at a sensible threshold: the index arithmetic lives here
+            auto scan_vec = [&](int v, const uint4& w) {
                 if (!vec_any(w)) return;
-                const int k = v / vpr, wv = v - k * vpr;
-                const unsigned ww[4] = {w.x, w.y, w.z, w.w};
-#pragma unroll
-                for (int i = 0; i < 4; ++i) {
-                    const int wi = 4 * wv + i;                 // word index within the row
-                    if (ACC16) {
-                        const unsigned a0 = ww[i] & 0xFFFFu, a1 = ww[i] >> 16;
-                        const int jl0 = 64 * (wi >> 5) + (wi & 31);
-                        if (a0 >= thr) candidate(jl0, k, a0);
-                        if (a1 >= thr) candidate(jl0 + 32, k, a1);
-                    } else {
-                        if (ww[i] >= thr) candidate(wi, k, ww[i]);   // word (2G+h)*32 + l IS column 64G + 32h + l
-                    }
-                }
+                const int pos = atomicAdd(&misc[42], 1);
+                if (pos < vcap) { vlist[pos] = (unsigned)v; return; }
+#pragma unroll 1
+                for (int c = 0; c < CELLS; ++c) test_cell(v, c);
             };
             int v = tid;
             for (; v + 3 * nthreads < n_vec; v += 4 * nthreads) {   // four vectors per trip, one test
@@ -430,12 +437,8 @@ __global__ void __launch_bounds__(1024, 1) hough_event_kernel(const __grid_const
             }
             for (; v < n_vec; v += nthreads) scan_vec(v, acc4[v]);
             __syncthreads();
-            const int n_cand = min(misc[42], cand_cap);
-            for (int i = tid; i < n_cand; i += nthreads) {
-                const unsigned id = cand[i];
-                const int jl = (int)(id & 0xFFFFu), kk = (int)(id >> 16);
-                test_peak(jl, kk, cell_from<ACC16>(acc, p.pitch_b, jl, kk));
-            }
+            const int n_items = min(misc[42], vcap) * CELLS;
+            for (int i = tid; i < n_items; i += nthreads) test_cell((int)vlist[i / CELLS], i % CELLS);
         }
         __syncthreads();
 

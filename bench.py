@@ -194,12 +194,17 @@ def hbm_peak():
 
 
 def dram_traffic(workload_name):
-    """dram__bytes_read.sum + dram__bytes_write.sum per launch of the kernel, from the committed ncu capture."""
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of the kernel, from the committed ncu capture
+    (profiles/dram_traffic.csv); None when this workload has no capture."""
     try:
-        with open(os.path.join(ROOT, "profiles", "dram_traffic.json")) as f:
-            return json.load(f).get(workload_name)
+        import csv
+        with open(os.path.join(ROOT, "profiles", "dram_traffic.csv")) as f:
+            for row in csv.DictReader(f):
+                if row["workload"] == workload_name:
+                    return int(row["dram_bytes_read_per_launch"]) + int(row["dram_bytes_write_per_launch"])
     except Exception:  # noqa: BLE001
-        return None
+        pass
+    return None
 
 
 def run_ours(args):
@@ -341,6 +346,11 @@ def run_ours(args):
         "peak_source": "hough_bench_shared_atomics(variant 5) measured in this run: conflict-free 32-bit shared atomics, all SMs",
         "algorithmic_votes_per_launch": v_in, "algorithmic_bytes_per_launch": alg_bytes,
         "t_vote_us": t_vote * 1e6, "t_hbm_us": t_hbm * 1e6, "t_kernel_us": t_kernel * 1e6,
+        # diagnostic third ceiling: 10.3 issue slots per (hit, theta) vote, 4 slots per clock per SM
+        "issue_slot_ceiling": {"slots_per_vote": 10.3, "peak": info["SM_COUNT"] * (clocks.get("sm_mhz") or 1965) * 1e6 * 128 / 10.3 / 1e9,
+                               "achieved": pairs / t_kernel / 1e9, "unit": "Gvotes/s (hit x theta)",
+                               "frac": (pairs / t_kernel) / (info["SM_COUNT"] * (clocks.get("sm_mhz") or 1965) * 1e6 * 128 / 10.3),
+                               "source": "profiles/r01_microbench_voteloop.md"},
         "hbm": {"achieved": alg_bytes / t_kernel / 1e9, "peak": hbm_gbs, "unit": "GB/s", "frac": t_hbm / t_kernel, "peak_source": hbm_src},
     }
 

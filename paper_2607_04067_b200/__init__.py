@@ -39,7 +39,7 @@ HOUGH_INFO_LAUNCHES = 10
 EXPORTS = [
     "hough_create", "hough_set_option", "hough_set_trig_table", "hough_get_info", "hough_run", "hough_run_ex",
     "hough_run_host", "hough_destroy", "hough_strerror", "hough_last_error", "hough_version",
-    "hough_bench_shared_atomics",
+    "hough_bench_shared_atomics", "hough_plan_describe",
 ]
 
 
@@ -92,6 +92,8 @@ def load_library():
     lib.hough_last_error.argtypes = []
     lib.hough_version.restype = ctypes.c_char_p
     lib.hough_version.argtypes = []
+    lib.hough_plan_describe.restype = ci
+    lib.hough_plan_describe.argtypes = [ci, ci, ci, ci, ci, ci, ctypes.POINTER(cll), ci]
     lib.hough_bench_shared_atomics.restype = ci
     lib.hough_bench_shared_atomics.argtypes = [ci, ci, ci, cll, ctypes.POINTER(ctypes.c_double)]
     _lib = lib
@@ -188,6 +190,19 @@ def hough_bench_shared_atomics(variant, ctas_per_sm, threads, iters):
     _check(load_library().hough_bench_shared_atomics(variant, ctas_per_sm, threads, iters, ctypes.byref(out)),
            "hough_bench_shared_atomics")
     return out.value
+
+
+PLAN_FIELDS = ("cluster_size", "threads", "smem_bytes", "acc_bits", "cols_per_lane", "cols_per_cta", "n_groups", "n_stripes",
+               "pitch_bytes", "bitmap_words_per_row", "chunk_hits", "region_bytes", "pbm_off", "pbm_bytes", "hb_off", "misc_off",
+               "w8_off", "w8_pitch", "mcf_off", "msf_off", "colq_off", "stash_off", "cnt_off", "gcnt_off", "rcp_groups", "rcp_2s")
+
+
+def hough_plan_describe(n_theta, n_rho, acc_dtype=HOUGH_ACC_AUTO, cluster_size=0, ctas_per_sm=0, smem_optin=0):
+    """Launch shape and shared-memory layout the library would choose (host-only, needs no GPU) as a dict."""
+    out = (ctypes.c_longlong * len(PLAN_FIELDS))()
+    _check(load_library().hough_plan_describe(n_theta, n_rho, acc_dtype, cluster_size, ctas_per_sm, smem_optin, out, len(PLAN_FIELDS)),
+           "hough_plan_describe")
+    return dict(zip(PLAN_FIELDS, [int(x) for x in out]))
 
 
 # ---------------------------------------------------------------- convenience wrapper (allocation + marshalling only)

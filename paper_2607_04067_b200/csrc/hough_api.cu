@@ -170,23 +170,26 @@ bool try_plan(const hough_ctx* c, bool acc16, int C, int want_ctas, Plan* out) {
     return true;
 }
 
-int make_plan(hough_ctx* c) {
+// Pure host logic (no CUDA call): the smallest cluster of {1,2,4,8} CTAs whose layout fits, two CTAs per SM if possible.
+bool choose_plan(const hough_ctx* c, Plan* best) {
     const bool acc16 = c->acc_dtype != HOUGH_ACC_U32;
     const int cands[4] = {1, 2, 4, 8};
-    Plan best;
-    bool found = false;
-    for (int ci = 0; ci < 4 && !found; ++ci) {
+    for (int ci = 0; ci < 4; ++ci) {
         const int C = cands[ci];
         if (c->opt_cluster && C != c->opt_cluster) continue;
         if (C > c->n_theta) continue;
         // prefer two CTAs per SM (phases of co-resident events overlap), else one
         const int first = (c->opt_ctas_per_sm == 1) ? 1 : 2;
-        for (int want = first; want >= 1 && !found; --want) {
-            Plan pl;
-            if (try_plan(c, acc16, C, want, &pl)) { best = pl; found = true; }
-        }
+        for (int want = first; want >= 1; --want)
+            if (try_plan(c, acc16, C, want, best)) return true;
     }
-    if (!found)
+    return false;
+}
+
+int make_plan(hough_ctx* c) {
+    const bool acc16 = c->acc_dtype != HOUGH_ACC_U32;
+    Plan best;
+    if (!choose_plan(c, &best))
         return fail(HOUGH_ERR_UNSUPPORTED, "a %d x %d %s accumulator does not fit the shared memory of %s",
                     c->n_theta, c->n_rho, acc16 ? "u16" : "u32",
                     c->opt_cluster ? "the requested cluster size" : "an 8-CTA cluster");
@@ -488,6 +491,29 @@ const char* hough_strerror(int status) {
 }
 
 const char* hough_last_error(void) { return g_err; }
+
+int hough_plan_describe(int n_theta, int n_rho, int acc_dtype, int cluster_size, int ctas_per_sm, int smem_optin,
+                        long long* out, int n_out) {
+    if (n_theta < 1 || n_theta > 65535 || n_rho < 1 || n_rho > 65535 || !out || n_out < HOUGH_PLAN_N_FIELDS)
+        return fail(HOUGH_ERR_INVALID_ARG, "bad argument");
+    if (acc_dtype != HOUGH_ACC_AUTO && acc_dtype != HOUGH_ACC_U16 && acc_dtype != HOUGH_ACC_U32) return fail(HOUGH_ERR_INVALID_ARG, "bad accumulator dtype");
+    if (cluster_size != 0 && cluster_size != 1 && cluster_size != 2 && cluster_size != 4 && cluster_size != 8)
+        return fail(HOUGH_ERR_INVALID_ARG, "cluster size must be 0,1,2,4,8");
+    if (ctas_per_sm < 0 || ctas_per_sm > 2) return fail(HOUGH_ERR_INVALID_ARG, "ctas_per_sm must be 0,1,2");
+    hough_ctx c;
+    c.n_theta = n_theta; c.n_rho = n_rho; c.threshold = 1; c.window = 0; c.rho_max = 1.0f; c.inv = 1.0f;
+    c.acc_dtype = acc_dtype; c.opt_cluster = cluster_size; c.opt_ctas_per_sm = ctas_per_sm;
+    c.smem_optin = smem_optin > 0 ? smem_optin : 232448;   // B200: 227 KB per CTA with opt-in
+    Plan pl;
+    if (!choose_plan(&c, &pl)) return fail(HOUGH_ERR_UNSUPPORTED, "the accumulator does not fit");
+    const KParams& k = pl.kp;
+    const long long v[HOUGH_PLAN_N_FIELDS] = {
+        pl.csize, pl.threads, pl.smem_bytes, pl.acc16 ? 16 : 32, pl.cpl, k.cols_per_cta, k.n_groups, k.n_stripes,
+        k.pitch_b, k.wpr, k.chunk, k.region_bytes, k.pbm_off, k.pbm_bytes, k.hb_off, k.misc_off,
+        k.w8_off, k.w8_pitch, k.mcf_off, k.msf_off, k.colq_off, k.stash_off, k.cnt_off, k.gcnt_off, k.rcp_groups, k.rcp_2s};
+    for (int i = 0; i < HOUGH_PLAN_N_FIELDS; ++i) out[i] = v[i];
+    return HOUGH_OK;
+}
 
 const char* hough_version(void) { return "hough-b200 0.1 (sm_100a)"; }
 

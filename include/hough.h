@@ -80,7 +80,7 @@ typedef enum hough_info {
     HOUGH_INFO_THREADS = 2,         /* threads per CTA */
     HOUGH_INFO_SMEM_BYTES = 3,      /* dynamic shared memory per CTA */
     HOUGH_INFO_CTAS_PER_SM = 4,     /* resident CTAs per SM (occupancy query) */
-    HOUGH_INFO_GRID_MAX = 5,        /* CTAs of a full persistent grid */
+    HOUGH_INFO_GRID_MAX = 5,        /* CTAs resident on the device at once (a launch has one CTA or cluster per event) */
     HOUGH_INFO_ACC_BITS = 6,        /* 16 or 32 */
     HOUGH_INFO_MAX_PEAKS = 7,
     HOUGH_INFO_CHUNK_HITS = 8,      /* hits staged in shared memory per pass */

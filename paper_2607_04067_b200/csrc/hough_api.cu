@@ -279,9 +279,10 @@ int launch(hough_ctx* c, const hough_io* io, cudaStream_t stream) {
     kp.force_slow = c->opt_vote_path == 1;
     kp.diag = c->opt_vote_path >= 2 ? c->opt_vote_path : 0;
     const int C = pl.csize;
+    // one CTA (cluster) per event: the hardware block scheduler deals events to the SM slots as they free up, which
+    // balances events of different size; the kernel's event loop only matters beyond 2^31 CTAs
     long long want = (long long)io->n_events * C;
-    const long long cap = getenv("HOUGH_PERSISTENT") ? (long long)pl.grid_max : 0x7FFFFFF0LL;
-    int grid = (int)std::min<long long>(want, cap);
+    int grid = (int)std::min<long long>(want, 0x7FFFFFF0LL);
     grid = grid / C * C;
     if (grid < C) grid = C;
     const void* fn = pick_kernel(pl.acc16, C > 1, pl.cpl);

@@ -1,8 +1,9 @@
 // hough_kernel.cuh -- the fused per-event kernel (sm_100a).
 //
 // One CTA (or one thread-block cluster of C CTAs that split the theta columns)
-// owns one event at a time and walks a static round-robin list of events
-// (persistent grid, no scratch, re-entrant across streams).  Per event:
+// per event: the launch has n_events * C CTAs and the hardware block scheduler
+// deals them to the SM slots (no scratch, re-entrant across streams; the event
+// loop below only iterates beyond 2^31 CTAs).  Per event:
 //   H0/H1 stage hits -> conformal (u,v) in shared memory   PAPER.md:52-57 Eq. (1)
 //   H2/H3 vote: lane = CPL theta columns, warp-uniform hit
 //   H4    threshold + 3x3 local maximum -> peak bitmap

@@ -102,8 +102,9 @@ __device__ __forceinline__ float2 conformal(float2 h, float scale) {
 //   rho = fl(fl(u*c) + fl(v*s)); t = fl(fl(rho + rho_max) * inv); y = t + 1.5*2^23 rounded toward -inf.
 // Returns the raw bits of y: (bits - HOUGH_MAGIC_BITS) as unsigned is < n_rho  <=>  0 <= t < n_rho, and
 // then it IS floor(t) -- for every input, including NaN/inf/huge.
-// (Packed fp32x2 instructions were measured on B200 to take two issue slots each, so they buy nothing
-// in this issue-bound loop and they invite FFMA2 contraction; profiles/r01_microbench.md.)
+// This scalar form is exact for ANY hit; selection (H6) uses it.  The voting loop uses the packed form below,
+// which takes the same number of issue slots (a packed fp32x2 instruction occupies two,
+// profiles/r01_microbench_voteloop.md) but half the instructions and registers.
 __device__ __forceinline__ unsigned bin_bits(float u, float v, float c, float s, float rho_max, float inv) {
     const float rho = __fadd_rn(__fmul_rn(u, c), __fmul_rn(v, s));
     const float t = __fmul_rn(__fadd_rn(rho, rho_max), inv);

@@ -68,9 +68,7 @@ typedef enum hough_option {
     HOUGH_OPT_CLUSTER_SIZE = 4,     /* 0 = smallest of {1,2,4,8} that fits (default), else force 1,2,4,8 */
     HOUGH_OPT_CTAS_PER_SM = 5,      /* 0 = as many as fit, up to 2 (default); tuning knob */
     HOUGH_OPT_VOTE_PATH = 6         /* 0 = fast voting with packed fp32x2 arithmetic, the exact slow path only for
-                                       degenerate hits (default); 1 = force the slow path (testing);
-                                       2, 3 = timing diagnostics whose OUTPUTS ARE UNDEFINED: 2 skips the voting loops,
-                                       3 skips everything after voting (bench.py --vote-path) */
+                                       degenerate hits (default); 1 = force the exact slow path everywhere (testing) */
 } hough_option;
 
 enum { HOUGH_ACC_AUTO = 0, HOUGH_ACC_U16 = 1, HOUGH_ACC_U32 = 2 };
@@ -102,8 +100,12 @@ hough_ctx* hough_create(int n_theta, int n_rho, float rho_max, int threshold, in
  * configuration does not fit the device. */
 int hough_set_option(hough_ctx* ctx, int key, long long value);
 
-/* Replaces the theta table: h_cos[j], h_sin[j], j < n_theta, HOST pointers,
- * copied (synchronously).  Values must be finite. */
+/* Replaces the theta table of the rho matrix R ("discrete
+ * angle theta_j", the cos/sin factors of PAPER.md:69): h_cos[j], h_sin[j],
+ * j < n_theta, HOST pointers, copied (synchronously).  Values must be finite.
+ * Lets a caller fix theta samples other than the default left bin edges
+ * (the paper does not say edge or centre, reading Q3) and hands the
+ * kernel the very table an external checker uses. */
 int hough_set_trig_table(hough_ctx* ctx, const float* h_cos, const float* h_sin);
 
 /* Reads a property of the current configuration (see hough_info); negative on error. */
@@ -124,7 +126,9 @@ long long hough_get_info(const hough_ctx* ctx, int key);
 int hough_run(hough_ctx* ctx, const float* d_xy, const int32_t* d_event_offsets, int n_events,
               uint8_t* d_keep_mask, hough_peak* d_peaks, int32_t* d_counts, hough_stream stream);
 
-/* hough_run plus optional outputs (any of the last three may be NULL):
+/* hough_run plus optional outputs (any of the last three may be NULL): the
+ * reduced hit set itself (the N_select hits of Eq. (8), that
+ * go on to track fitting) and the accumulator of PAPER.md:96-104:
  *   d_kept_xy    [n_total][2] fp32 and
  *   d_kept_idx   [n_total] int32: event e's kept hits, in original order, start
  *                at d_event_offsets[e]; kept_idx is the index within the event;
@@ -145,12 +149,19 @@ typedef struct hough_io {
 
 int hough_run_ex(hough_ctx* ctx, const hough_io* io, hough_stream stream);
 
-/* End-to-end form with HOST buffers (pinned memory recommended): copies
+/* End-to-end form with HOST buffers (pinned memory recommended), the shape of
+ * the paper's own measurement: events are "transmitted to the GPU memory" in
+ * batches and "only the extracted peak results need to be returned"
+ * (PAPER.md:90, :106).  Copies
  * h_xy / h_event_offsets to a library-owned device staging area, runs H0-H7
  * and copies keep mask, peaks and counts (and kept_xy / kept_idx when not
  * NULL) back, all asynchronously on `stream`; the host outputs are valid after
- * the caller synchronises `stream`.  NOT re-entrant (the staging area belongs
- * to the handle) and may allocate when a batch is larger than any before. */
+ * the caller synchronises `stream`.  h_kept_xy / h_kept_idx NULL = lean mode:
+ * only mask, peaks and counts come back (a host consumer that still holds h_xy
+ * can compact by the mask).  Only the entries hough_run defines are meaningful;
+ * the rest of h_peaks and of the kept arrays is zero.  NOT re-entrant (the
+ * staging area belongs to the handle) and may allocate when a batch is larger
+ * than any before. */
 int hough_run_host(hough_ctx* ctx, const float* h_xy, const int32_t* h_event_offsets, int n_events,
                    uint8_t* h_keep_mask, hough_peak* h_peaks, int32_t* h_counts,
                    float* h_kept_xy, int32_t* h_kept_idx, hough_stream stream);
@@ -161,39 +172,6 @@ void hough_destroy(hough_ctx* ctx);
 const char* hough_strerror(int status);
 const char* hough_last_error(void);      /* thread-local message of the last failure */
 const char* hough_version(void);
-
-/* Measurement aid (the denominator of the vote roofline): times a
- * kernel that does nothing but `iters` conflict-free no-return 32-bit shared
- * atomic adds per thread, with `ctas_per_sm` x `threads` resident per SM, and
- * returns atomics per second over the whole device in *out_rate.
- *   variant 0: every lane its own bank, add of 1 (ATOMS.POPC.INC)
- *   variant 1: every lane its own bank, add of a register value (ATOMS.ADD)
- *   variant 2: pseudo-random bank per lane (natural bank conflicts)
- *   variant 3: the voting loop's instruction mix without the atomics (issue bound)
- *   variant 4: the voting loop's instruction mix with conflict-free atomics
- *   variant 5: the ATOMS pipe alone: eight fixed conflict-free addresses per thread, no address
- *              arithmetic in the loop (the peak the vote roofline divides by)
- *   variant 6: variant 3 with packed fp32x2 arithmetic;  variant 7: variant 4 with packed arithmetic
- *   variant 8: variant 7 with a 512-byte (power of two) row pitch
- *   (variants 3, 4, 6-8 report lane-votes per second, padded lanes included)
- * Synchronises the device. */
-int hough_bench_shared_atomics(int variant, int ctas_per_sm, int threads, long long iters, double* out_rate);
-
-/* Host-only introspection (needs NO CUDA device): the launch shape and shared-memory layout the library would
- * choose for an n_theta x n_rho accumulator of `acc_dtype` (HOUGH_ACC_*), with `cluster_size` / `ctas_per_sm` as in
- * hough_set_option (0 = automatic) on a device with `smem_optin` bytes of opt-in shared memory per CTA (0 = B200's
- * 232448).  Writes HOUGH_PLAN_N_FIELDS values to out[] in the order of enum hough_plan_field; n_out must be at
- * least that.  HOUGH_ERR_UNSUPPORTED if nothing fits.  Used by the CPU tests of the planner. */
-enum { HOUGH_PLAN_N_FIELDS = 26 };
-typedef enum hough_plan_field {
-    HOUGH_PLAN_CLUSTER_SIZE = 0, HOUGH_PLAN_THREADS, HOUGH_PLAN_SMEM_BYTES, HOUGH_PLAN_ACC_BITS, HOUGH_PLAN_COLS_PER_LANE,
-    HOUGH_PLAN_COLS_PER_CTA, HOUGH_PLAN_N_GROUPS, HOUGH_PLAN_N_STRIPES, HOUGH_PLAN_PITCH_BYTES, HOUGH_PLAN_BITMAP_WORDS_PER_ROW,
-    HOUGH_PLAN_CHUNK_HITS, HOUGH_PLAN_REGION_BYTES, HOUGH_PLAN_PBM_OFF, HOUGH_PLAN_PBM_BYTES, HOUGH_PLAN_HB_OFF, HOUGH_PLAN_MISC_OFF,
-    HOUGH_PLAN_W8_OFF, HOUGH_PLAN_W8_PITCH, HOUGH_PLAN_MCF_OFF, HOUGH_PLAN_MSF_OFF, HOUGH_PLAN_COLQ_OFF, HOUGH_PLAN_STASH_OFF,
-    HOUGH_PLAN_CNT_OFF, HOUGH_PLAN_GCNT_OFF, HOUGH_PLAN_RCP_GROUPS, HOUGH_PLAN_RCP_2S
-} hough_plan_field;
-int hough_plan_describe(int n_theta, int n_rho, int acc_dtype, int cluster_size, int ctas_per_sm, int smem_optin,
-                        long long* out, int n_out);
 
 #ifdef __cplusplus
 }

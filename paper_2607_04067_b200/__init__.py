@@ -36,11 +36,13 @@ HOUGH_INFO_CHUNK_HITS = 8
 HOUGH_INFO_SM_COUNT = 9
 HOUGH_INFO_LAUNCHES = 10
 
-EXPORTS = [
+# what each header under include/ declares, and which library exports it
+EXPORTS = [            # include/hough.h -> libhough_b200.so (the product ABI)
     "hough_create", "hough_set_option", "hough_set_trig_table", "hough_get_info", "hough_run", "hough_run_ex",
     "hough_run_host", "hough_destroy", "hough_strerror", "hough_last_error", "hough_version",
-    "hough_bench_shared_atomics", "hough_plan_describe",
 ]
+DEBUG_EXPORTS = ["hough_plan_describe", "hough_debug_tame_bounds", "hough_debug_bounds_enabled"]   # include/hough_debug.h, same library
+BENCH_EXPORTS = ["hough_bench_shared_atomics", "hough_bench_vote_loop", "hough_bench_issue_rate"]   # include/hough_bench.h -> libhough_bench.so
 
 
 class hough_io(ctypes.Structure):
@@ -56,10 +58,20 @@ class HoughError(RuntimeError):
 
 
 _lib = None
+_bench_lib = None
+
+
+def flavor() -> str:
+    """Which build of the product library this process uses: "release" (default), "dbg" (every shared-memory
+    offset checked, HOUGH_B200_FLAVOR=dbg) or "diag" (bench-only phase-skipping diagnostics)."""
+    f = os.environ.get("HOUGH_B200_FLAVOR", "release")
+    if f not in ("release", "dbg", "diag"):
+        raise HoughError("HOUGH_B200_FLAVOR must be release, dbg or diag (got %r)" % f)
+    return f
 
 
 def lib_path() -> str:
-    return _build.LIB
+    return _build.lib_path(flavor())
 
 
 def load_library():
@@ -67,7 +79,7 @@ def load_library():
     global _lib
     if _lib is not None:
         return _lib
-    path = _build.build()
+    path = _build.build(flavor())
     lib = ctypes.CDLL(path)
     vp, ci, cll = ctypes.c_void_p, ctypes.c_int, ctypes.c_longlong
     lib.hough_create.restype = vp
@@ -94,9 +106,28 @@ def load_library():
     lib.hough_version.argtypes = []
     lib.hough_plan_describe.restype = ci
     lib.hough_plan_describe.argtypes = [ci, ci, ci, ci, ci, ci, ctypes.POINTER(cll), ci]
-    lib.hough_bench_shared_atomics.restype = ci
-    lib.hough_bench_shared_atomics.argtypes = [ci, ci, ci, cll, ctypes.POINTER(ctypes.c_double)]
+    lib.hough_debug_tame_bounds.restype = ci
+    lib.hough_debug_tame_bounds.argtypes = [ci, ctypes.c_float, ctypes.c_float, ctypes.c_float, ctypes.POINTER(ctypes.c_float)]
+    lib.hough_debug_bounds_enabled.restype = ci
+    lib.hough_debug_bounds_enabled.argtypes = []
     _lib = lib
+    return lib
+
+
+def load_bench_library():
+    """Loads libhough_bench.so (measurement aids, include/hough_bench.h); not needed by the product path."""
+    global _bench_lib
+    if _bench_lib is not None:
+        return _bench_lib
+    lib = ctypes.CDLL(_build.build("bench"))
+    ci, cll, pd = ctypes.c_int, ctypes.c_longlong, ctypes.POINTER(ctypes.c_double)
+    lib.hough_bench_shared_atomics.restype = ci
+    lib.hough_bench_shared_atomics.argtypes = [ci, ci, ci, cll, pd]
+    lib.hough_bench_vote_loop.restype = ci
+    lib.hough_bench_vote_loop.argtypes = [ci, ci, ci, ci, cll, pd]
+    lib.hough_bench_issue_rate.restype = ci
+    lib.hough_bench_issue_rate.argtypes = [ci, ci, ci, cll, pd]
+    _bench_lib = lib
     return lib
 
 
@@ -156,14 +187,57 @@ def hough_get_info(ctx, key):
     return int(load_library().hough_get_info(ctx, key))
 
 
+def _marshal_check(cuda, n_events, xy, off, keep, peaks, counts, kept_xy=None, kept_idx=None, accum=None, max_peaks=None,
+                   grid=None):
+    """Marshalling-side sanity of the buffers handed to the C ABI (dtype, device, contiguity, length): the library
+    itself only sees raw pointers.  No arithmetic of the method."""
+    import torch
+    def chk(name, t, dtype, min_numel):
+        if t is None:
+            return
+        if not isinstance(t, torch.Tensor):
+            raise HoughError("%s must be a torch tensor" % name)
+        if t.dtype != dtype:
+            raise HoughError("%s must be %s (got %s)" % (name, dtype, t.dtype))
+        if t.is_cuda != cuda:
+            raise HoughError("%s must be a %s tensor" % (name, "CUDA" if cuda else "host"))
+        if not t.is_contiguous():
+            raise HoughError("%s must be contiguous" % name)
+        if t.numel() < min_numel:
+            raise HoughError("%s holds %d elements, needs at least %d" % (name, t.numel(), min_numel))
+    if n_events <= 0:
+        return
+    chk("event offsets", off, torch.int32, n_events + 1)
+    if off is None or xy is None:
+        return                         # the C ABI reports the null pointer
+    n_total = xy.numel() // 2
+    chk("xy", xy, torch.float32, 0)
+    chk("keep mask", keep, torch.uint8, n_total)
+    chk("counts", counts, torch.int32, 2 * n_events)
+    if max_peaks:
+        chk("peaks", peaks, torch.int32, 2 * n_events * max_peaks)
+    chk("kept_xy", kept_xy, torch.float32, 2 * n_total)
+    chk("kept_idx", kept_idx, torch.int32, n_total)
+    if accum is not None and grid is not None:
+        chk("accum dump", accum, torch.int32, n_events * grid[0] * grid[1])
+    if cuda:
+        devs = {t.device for t in (xy, off, keep, peaks, counts, kept_xy, kept_idx, accum) if t is not None and t.numel()}
+        if len(devs) > 1:
+            raise HoughError("all tensors must live on one device (got %s)" % sorted(map(str, devs)))
+
+
 def hough_run(ctx, d_xy, d_event_offsets, n_events, d_keep_mask, d_peaks, d_counts, stream=None):
     """Tensors are CUDA torch tensors (see include/hough.h for shapes); asynchronous on `stream`."""
+    _marshal_check(True, n_events, d_xy, d_event_offsets, d_keep_mask, d_peaks, d_counts,
+                   max_peaks=hough_get_info(ctx, HOUGH_INFO_MAX_PEAKS))
     _check(load_library().hough_run(ctx, _ptr(d_xy), _ptr(d_event_offsets), n_events, _ptr(d_keep_mask),
                                     _ptr(d_peaks), _ptr(d_counts), _stream_handle(stream)), "hough_run")
 
 
 def hough_run_ex(ctx, d_xy, d_event_offsets, n_events, d_keep_mask, d_peaks, d_counts,
                  d_kept_xy=None, d_kept_idx=None, d_accum_dump=None, stream=None):
+    _marshal_check(True, n_events, d_xy, d_event_offsets, d_keep_mask, d_peaks, d_counts, d_kept_xy, d_kept_idx,
+                   max_peaks=hough_get_info(ctx, HOUGH_INFO_MAX_PEAKS))
     io = hough_io(_ptr(d_xy), _ptr(d_event_offsets), n_events, _ptr(d_keep_mask), _ptr(d_peaks), _ptr(d_counts),
                   _ptr(d_kept_xy), _ptr(d_kept_idx), _ptr(d_accum_dump))
     _check(load_library().hough_run_ex(ctx, ctypes.byref(io), _stream_handle(stream)), "hough_run_ex")
@@ -172,6 +246,8 @@ def hough_run_ex(ctx, d_xy, d_event_offsets, n_events, d_keep_mask, d_peaks, d_c
 def hough_run_host(ctx, h_xy, h_event_offsets, n_events, h_keep_mask, h_peaks, h_counts,
                    h_kept_xy=None, h_kept_idx=None, stream=None):
     """HOST (ideally pinned) torch tensors in and out; copies are inside the call, asynchronous on `stream`."""
+    _marshal_check(False, n_events, h_xy, h_event_offsets, h_keep_mask, h_peaks, h_counts, h_kept_xy, h_kept_idx,
+                   max_peaks=hough_get_info(ctx, HOUGH_INFO_MAX_PEAKS))
     _check(load_library().hough_run_host(ctx, _ptr(h_xy), _ptr(h_event_offsets), n_events, _ptr(h_keep_mask),
                                          _ptr(h_peaks), _ptr(h_counts), _ptr(h_kept_xy), _ptr(h_kept_idx),
                                          _stream_handle(stream)), "hough_run_host")
@@ -185,11 +261,39 @@ def hough_version():
     return load_library().hough_version().decode()
 
 
-def hough_bench_shared_atomics(variant, ctas_per_sm, threads, iters):
+def _bench_call(name, *args):
     out = ctypes.c_double(0.0)
-    _check(load_library().hough_bench_shared_atomics(variant, ctas_per_sm, threads, iters, ctypes.byref(out)),
-           "hough_bench_shared_atomics")
+    rc = getattr(load_bench_library(), name)(*args, ctypes.byref(out))
+    if rc != 0:
+        raise HoughError("%s failed with status %d%s" % (name, rc, " (no CUDA device?)" if rc == -3 else ""))
     return out.value
+
+
+def hough_bench_shared_atomics(variant, ctas_per_sm, threads, iters):
+    """Shared atomics per second over the whole device (include/hough_bench.h); variant 5 = the roofline's peak."""
+    return _bench_call("hough_bench_shared_atomics", variant, ctas_per_sm, threads, iters)
+
+
+def hough_bench_vote_loop(mode, cpl, ctas_per_sm, threads, iters):
+    """Lane-votes per second of the voting loop's instruction mix (include/hough_bench.h)."""
+    return _bench_call("hough_bench_vote_loop", mode, cpl, ctas_per_sm, threads, iters)
+
+
+def hough_bench_issue_rate(kind, ctas_per_sm, threads, iters):
+    """Warp-instructions per second of one instruction class (include/hough_bench.h)."""
+    return _bench_call("hough_bench_issue_rate", kind, ctas_per_sm, threads, iters)
+
+
+def hough_debug_tame_bounds(n_rho, rho_max, table_max, table_min_nz):
+    """(tame_bound, ftz_min) as the kernel receives them (include/hough_debug.h); host-only."""
+    out = (ctypes.c_float * 2)()
+    _check(load_library().hough_debug_tame_bounds(n_rho, ctypes.c_float(rho_max), ctypes.c_float(table_max),
+                                                  ctypes.c_float(table_min_nz), out), "hough_debug_tame_bounds")
+    return float(out[0]), float(out[1])
+
+
+def hough_debug_bounds_enabled():
+    return bool(load_library().hough_debug_bounds_enabled())
 
 
 PLAN_FIELDS = ("cluster_size", "threads", "smem_bytes", "acc_bits", "cols_per_lane", "cols_per_cta", "n_groups", "n_stripes",

@@ -7,9 +7,13 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <map>
+#include <mutex>
 #include <new>
+#include <utility>
 #include <vector>
 
+#include "../../include/hough_debug.h"
 #include "hough_kernel.cuh"
 
 using hough::KParams;
@@ -92,6 +96,19 @@ const void* kernel_ptr(int cpl) {
 const void* pick_kernel(bool acc16, bool cl, int cpl) {
     if (acc16) return cl ? kernel_ptr<true, true>(cpl) : kernel_ptr<true, false>(cpl);
     return cl ? kernel_ptr<false, true>(cpl) : kernel_ptr<false, false>(cpl);
+}
+
+// cudaFuncAttributeMaxDynamicSharedMemorySize belongs to the kernel (per device), not to a handle: several live
+// handles may share one instantiation with different footprints, so the attribute is only ever RAISED.
+int raise_smem_limit(int device, const void* fn, int bytes) {
+    static std::mutex mu;
+    static std::map<std::pair<int, const void*>, int> high;
+    std::lock_guard<std::mutex> lk(mu);
+    int& h = high[std::make_pair(device, fn)];
+    if (bytes <= h) return HOUGH_OK;
+    CUDA_TRY(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
+    h = bytes;
+    return HOUGH_OK;
 }
 
 // Lays out shared memory for cluster size C and `want_ctas` CTAs per SM.  Returns false if it does not fit.
@@ -194,7 +211,10 @@ int make_plan(hough_ctx* c) {
                     c->n_theta, c->n_rho, acc16 ? "u16" : "u32",
                     c->opt_cluster ? "the requested cluster size" : "an 8-CTA cluster");
     const void* fn = pick_kernel(best.acc16, best.csize > 1, best.cpl);
-    CUDA_TRY(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, best.smem_bytes));
+    int cur = -1;
+    CUDA_TRY(cudaGetDevice(&cur));
+    if (cur != c->device) return fail(HOUGH_ERR_INVALID_ARG, "the handle belongs to device %d but device %d is current", c->device, cur);
+    if (int rc = raise_smem_limit(c->device, fn, best.smem_bytes)) return rc;
     int occ = 0;
     if (best.csize == 1) {
         CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fn, best.threads, best.smem_bytes));
@@ -238,27 +258,30 @@ int upload_table(hough_ctx* c, const float* h_cos, const float* h_sin) {
     return HOUGH_OK;
 }
 
-float tame_bound(const hough_ctx* c) {
+float tame_bound(float inv, float rho_max, float tmax) {
     // hits with (|u|+|v|) * tmax <= 0.99 * (2^17/inv - rho_max) have |t| < 2^17 at every column
-    double rho_lim = 131072.0 / (double)c->inv - (double)c->rho_max;
+    double rho_lim = 131072.0 / (double)inv - (double)rho_max;
     if (!(rho_lim > 0.0)) return 0.0f;
-    if (c->tmax <= 0.0f) return 3.0e38f;
-    double b = 0.99 * rho_lim / (double)c->tmax;
+    if (tmax <= 0.0f) return 3.0e38f;
+    double b = 0.99 * rho_lim / (double)tmax;
     return b > 3.0e38 ? 3.0e38f : (float)b;
 }
 
-float ftz_min(const hough_ctx* c) {
+float ftz_min(float tmin_nz) {
     // |u| >= 2^-125 / tmin_nz  =>  |u * c_j| >= 2^-125 (before rounding) for every non-zero table entry:
     // the product is a normal number and the .ftz of the packed multiply never acts.  Never below 2^-125,
     // so that a subnormal u or v (flushed on input) is excluded too.
-    if (!(c->tmin_nz > 0.0f) || !std::isfinite(c->tmin_nz)) return 2.3509887e-38f;   // all-zero table: nothing to flush
-    double b = std::ldexp(1.0, -125) / (double)c->tmin_nz;
+    if (!(tmin_nz > 0.0f) || !std::isfinite(tmin_nz)) return 2.3509887e-38f;   // all-zero table: nothing to flush
+    double b = std::ldexp(1.0, -125) / (double)tmin_nz;
     if (b < std::ldexp(1.0, -125)) b = std::ldexp(1.0, -125);
     return b > 3.0e38 ? 3.0e38f : (float)(b * 1.0000002);
 }
 
 int launch(hough_ctx* c, const hough_io* io, cudaStream_t stream) {
     const Plan& pl = c->plan;
+    int cur = -1;
+    if (cudaGetDevice(&cur) != cudaSuccess || cur != c->device)   // tables and kernel attributes are per device
+        return fail(HOUGH_ERR_INVALID_ARG, "the handle belongs to device %d but device %d is current", c->device, cur);
     KParams kp = pl.kp;
     kp.xy = (const float2*)io->d_xy;
     kp.off = io->d_event_offsets;
@@ -274,10 +297,12 @@ int launch(hough_ctx* c, const hough_io* io, cudaStream_t stream) {
     kp.n_theta = c->n_theta; kp.n_rho = c->n_rho; kp.threshold = c->threshold; kp.window = c->window;
     kp.max_peaks = c->max_peaks;
     kp.rho_max = c->rho_max; kp.inv = c->inv; kp.scale = (float)c->conformal_scale;
-    kp.tame_bound = tame_bound(c);
-    kp.ftz_min = ftz_min(c);
+    kp.tame_bound = tame_bound(c->inv, c->rho_max, c->tmax);
+    kp.ftz_min = ftz_min(c->tmin_nz);
     kp.force_slow = c->opt_vote_path == 1;
+#ifdef HOUGH_DIAG
     kp.diag = c->opt_vote_path >= 2 ? c->opt_vote_path : 0;
+#endif
     const int C = pl.csize;
     // one CTA (cluster) per event: the hardware block scheduler deals events to the SM slots as they free up, which
     // balances events of different size; the kernel's event loop only matters beyond 2^31 CTAs
@@ -371,7 +396,11 @@ int hough_set_option(hough_ctx* c, int key, long long value) {
             if (value < 0 || value > 2) return fail(HOUGH_ERR_INVALID_ARG, "ctas_per_sm must be 0,1,2");
             c->opt_ctas_per_sm = (int)value; break;
         case HOUGH_OPT_VOTE_PATH:
+#ifdef HOUGH_DIAG   // bench-only build: 2 skips the voting loops, 3 skips everything after voting (outputs undefined)
             if (value < 0 || value > 3) return fail(HOUGH_ERR_INVALID_ARG, "vote path must be 0..3");
+#else
+            if (value < 0 || value > 1) return fail(HOUGH_ERR_INVALID_ARG, "vote path must be 0 or 1");
+#endif
             c->opt_vote_path = (int)value; return HOUGH_OK;
         default:
             return fail(HOUGH_ERR_INVALID_ARG, "unknown option %d", key);
@@ -435,7 +464,7 @@ int hough_run_host(hough_ctx* c, const float* h_xy, const int32_t* h_off, int n_
     cudaStream_t st = (cudaStream_t)stream;
     const long long n_peaks_cap = (long long)n_events * c->max_peaks;
     if (n_total > c->cap_hits || n_events > c->cap_events || n_peaks_cap > c->cap_peaks) {
-        CUDA_TRY(cudaStreamSynchronize(st));
+        CUDA_TRY(cudaDeviceSynchronize());   // earlier copies on ANY stream may still use the old staging area
         cudaFree(c->s_xy); cudaFree(c->s_off); cudaFree(c->s_keep); cudaFree(c->s_peaks); cudaFree(c->s_counts);
         cudaFree(c->s_kept_xy); cudaFree(c->s_kept_idx);
         c->s_xy = nullptr; c->s_off = nullptr; c->s_keep = nullptr; c->s_peaks = nullptr; c->s_counts = nullptr;
@@ -455,6 +484,10 @@ int hough_run_host(hough_ctx* c, const float* h_xy, const int32_t* h_off, int n_
             return fail(HOUGH_ERR_NOMEM, "cudaMalloc of the staging area failed");
         }
     }
+    // the kernel leaves peak entries past n_stored and kept entries past n_kept untouched: zero what goes back
+    if (c->max_peaks > 0) CUDA_TRY(cudaMemsetAsync(c->s_peaks, 0, sizeof(hough_peak) * (size_t)n_peaks_cap, st));
+    if (h_kept_xy && n_total > 0) CUDA_TRY(cudaMemsetAsync(c->s_kept_xy, 0, sizeof(float) * 2 * n_total, st));
+    if (h_kept_idx && n_total > 0) CUDA_TRY(cudaMemsetAsync(c->s_kept_idx, 0, sizeof(int32_t) * n_total, st));
     if (n_total > 0) CUDA_TRY(cudaMemcpyAsync(c->s_xy, h_xy, sizeof(float) * 2 * n_total, cudaMemcpyHostToDevice, st));
     CUDA_TRY(cudaMemcpyAsync(c->s_off, h_off, sizeof(int32_t) * ((size_t)n_events + 1), cudaMemcpyHostToDevice, st));
     hough_io io{};
@@ -516,6 +549,28 @@ int hough_plan_describe(int n_theta, int n_rho, int acc_dtype, int cluster_size,
     return HOUGH_OK;
 }
 
-const char* hough_version(void) { return "hough-b200 0.1 (sm_100a)"; }
+int hough_debug_tame_bounds(int n_rho, float rho_max, float table_max, float table_min_nz, float* out2) {
+    if (n_rho < 1 || !(rho_max > 0.0f) || !out2) return fail(HOUGH_ERR_INVALID_ARG, "bad argument");
+    const float inv = (float)((double)n_rho / (2.0 * (double)rho_max));
+    out2[0] = tame_bound(inv, rho_max, table_max);
+    out2[1] = ftz_min(table_min_nz);
+    return HOUGH_OK;
+}
+
+int hough_debug_bounds_enabled(void) {
+#ifdef HOUGH_DEBUG_BOUNDS
+    return 1;
+#else
+    return 0;
+#endif
+}
+
+const char* hough_version(void) {
+#ifdef HOUGH_DEBUG_BOUNDS
+    return "hough-b200 0.2 (sm_100a, debug bounds)";
+#else
+    return "hough-b200 0.2 (sm_100a)";
+#endif
+}
 
 }  // extern "C"

@@ -41,6 +41,18 @@ typedef unsigned long long ull;
 #define HOUGH_MAGIC_BITS 0x4B400000u
 #define HOUGH_SEL_ROUND_BLOCKS 32   // clustered selection: hit blocks per CTA per round
 
+// -DHOUGH_DEBUG_BOUNDS (libhough_b200_dbg.so, paper_2607_04067_b200/build.py): every shared-memory offset of the
+// vote, H4, H5, H6 and H7 phases (and the compaction's global index) is checked against the plan's region sizes
+// before use.  A violating access is SKIPPED (never performed, never traps) and the event's d_counts entry becomes
+// {HOUGH_DBG_SENTINEL, phase}.  The release build compiles the checks away.
+#define HOUGH_DBG_SENTINEL (-2)
+enum { HB_STAGE = 1, HB_VOTE_FAST = 2, HB_VOTE_SLOW = 3, HB_H4 = 4, HB_H5 = 5, HB_H6_SETUP = 6, HB_KEEP = 7, HB_H7 = 8 };
+#ifdef HOUGH_DEBUG_BOUNDS
+#define HB_CHK(ok, phase) ((ok) ? true : ((dbg_viol = dbg_viol ? dbg_viol : (phase)), false))
+#else
+#define HB_CHK(ok, phase) (true)
+#endif
+
 struct KParams {
     const float2* xy;
     const int* off;
@@ -58,7 +70,9 @@ struct KParams {
     float tame_bound;     // a hit is "tame" iff (|u|+|v|) <= tame_bound (then |t| < 2^17 at every column) ...
     float ftz_min;        // ... and u, v are each 0 or >= ftz_min in magnitude (then no product u*c, v*s is subnormal)
     int force_slow;       // 1: literal slow path for every hit
-    int diag;             // timing diagnostics (outputs undefined): 2 = skip the vote loops, 3 = skip everything after voting
+#ifdef HOUGH_DIAG
+    int diag;             // bench-only build: 2 = skip the vote loops, 3 = skip everything after voting (outputs undefined)
+#endif
     int csize;            // CTAs per event (cluster size)
     int cols_per_cta;     // theta columns owned by one CTA
     int n_groups;         // groups of 32*CPL columns per CTA
@@ -249,6 +263,10 @@ __global__ void __launch_bounds__(1024, 1) hough_event_kernel(const __grid_const
         }
 
         const bool single = n <= p.chunk;    // the whole event is staged at once: (u,v) stay in hb until selection
+        int dbg_viol = 0;                    // HOUGH_DEBUG_BOUNDS: first phase whose offset check failed (else unused)
+        (void)dbg_viol;
+        const unsigned acc_end = (unsigned)(p.n_rho + 1) * (unsigned)p.pitch_b;   // accumulator incl. the trash row
+        (void)acc_end;
 
         // the first two hits of this thread are requested before the zeroing stores, which then overlap the latency
         float2 pre0 = make_float2(1.0f, 0.0f), pre1 = pre0;
@@ -273,7 +291,7 @@ __global__ void __launch_bounds__(1024, 1) hough_event_kernel(const __grid_const
                 else if (cbeg == 0 && i == tid + nthreads) h = pre1;
                 else h = __ldg(&p.xy[beg + cbeg + i]);
                 float2 uv = conformal(h, p.scale);
-                hb[i] = uv;
+                if (HB_CHK(i < p.chunk, HB_STAGE)) hb[i] = uv;
                 const float au = fabsf(uv.x), av = fabsf(uv.y);
                 tame &= (__fadd_rn(au, av) <= p.tame_bound) ? 1 : 0;                        // false for NaN/inf
                 tame &= ((au >= p.ftz_min || au == 0.0f) && (av >= p.ftz_min || av == 0.0f)) ? 1 : 0;
@@ -284,8 +302,11 @@ __global__ void __launch_bounds__(1024, 1) hough_event_kernel(const __grid_const
             // control flow (shared-window base in a uniform register, ATOMS [R+UR] addressing).
             const int S = p.n_stripes;
             const int R = (int)(((unsigned)m * p.rcp_2s) >> 20);   // m / (2 * S)
+#ifdef HOUGH_DIAG
             if (p.diag == 2) {
-            } else if (all_tame) {
+            } else
+#endif
+            if (all_tame) {
                 // out-of-range votes (rel >= limit, including every wrapped negative) land in the lane's own
                 // word of the trash row: no predicate, no branch, no conflict
                 auto vote_hit = [&](const float2 uv) {
@@ -296,11 +317,11 @@ __global__ void __launch_bounds__(1024, 1) hough_event_kernel(const __grid_const
                         const unsigned rel0 = min(b0 * pitch + lc0, trash0);
                         const unsigned rel1 = min(b1 * pitch + lc0, trash0);
                         if (ACC16) {
-                            atomicAdd((unsigned*)(acc + rel0 + 128 * (q / 2)), 1u);
-                            atomicAdd((unsigned*)(acc + rel1 + 128 * (q / 2)), 0x10000u);
+                            if (HB_CHK(rel0 + 128 * (q / 2) + 4 <= acc_end, HB_VOTE_FAST)) atomicAdd((unsigned*)(acc + rel0 + 128 * (q / 2)), 1u);
+                            if (HB_CHK(rel1 + 128 * (q / 2) + 4 <= acc_end, HB_VOTE_FAST)) atomicAdd((unsigned*)(acc + rel1 + 128 * (q / 2)), 0x10000u);
                         } else {
-                            atomicAdd((unsigned*)(acc + rel0 + 128 * q), 1u);
-                            atomicAdd((unsigned*)(acc + rel1 + 128 * (q + 1)), 1u);
+                            if (HB_CHK(rel0 + 128 * q + 4 <= acc_end, HB_VOTE_FAST)) atomicAdd((unsigned*)(acc + rel0 + 128 * q), 1u);
+                            if (HB_CHK(rel1 + 128 * (q + 1) + 4 <= acc_end, HB_VOTE_FAST)) atomicAdd((unsigned*)(acc + rel1 + 128 * (q + 1)), 1u);
                         }
                     }
                 };
@@ -318,7 +339,7 @@ __global__ void __launch_bounds__(1024, 1) hough_event_kernel(const __grid_const
                         const int jl = 32 * (g * CPL + q) + lane;
                         if (jl >= ncols) continue;
                         const int k = bin_exact(uv.x, uv.y, p.cos_t[col0 + jl], p.sin_t[col0 + jl], p.rho_max, p.inv, p.n_rho);
-                        if (k >= 0)
+                        if (k >= 0 && HB_CHK((unsigned)k * pitch + 4u * cell_word_off<ACC16>(jl) + 4 <= limit, HB_VOTE_SLOW))
                             red_shared_add(acc_s + (unsigned)k * pitch + 4u * cell_word_off<ACC16>(jl), (ACC16 && (q & 1)) ? 0x10000u : 1u);
                     }
                 }
@@ -328,7 +349,9 @@ __global__ void __launch_bounds__(1024, 1) hough_event_kernel(const __grid_const
         if (n == 0) __syncthreads();         // no staging barrier ran: order the zeroing before the scan
         if (CL) cg::this_cluster().sync();   // (A) every CTA's columns are complete
 
+#ifdef HOUGH_DIAG
         if (p.diag == 3) { __syncthreads(); continue; }
+#endif
 
         // ---- optional accumulator dump (parity / debugging; never timed)
         if (p.accum_dump) {
@@ -336,7 +359,7 @@ __global__ void __launch_bounds__(1024, 1) hough_event_kernel(const __grid_const
             const int cells = ncols * p.n_rho;
             for (int idx = tid; idx < cells; idx += nthreads) {
                 int jl = idx / p.n_rho, k = idx - jl * p.n_rho;
-                dst[idx] = cell_from<ACC16>(acc, p.pitch_b, jl, k);
+                if (HB_CHK((unsigned)k * pitch + 4u * cell_word_off<ACC16>(jl) + 4 <= limit, HB_H4)) dst[idx] = cell_from<ACC16>(acc, p.pitch_b, jl, k);
             }
         }
 
@@ -363,9 +386,11 @@ __global__ void __launch_bounds__(1024, 1) hough_event_kernel(const __grid_const
                     }
                     const unsigned char* colp = base + 4u * cell_word_off<ACC16>(jcl);
                     const int sh = ACC16 ? 16 * ((jcl >> 5) & 1) : 0;
-                    const unsigned w0 = *(const unsigned*)(colp + (size_t)km * p.pitch_b);
-                    const unsigned w1 = *(const unsigned*)(colp + (size_t)k * p.pitch_b);
-                    const unsigned w2 = *(const unsigned*)(colp + (size_t)kp1 * p.pitch_b);
+                    const bool in = HB_CHK(jcl >= 0 && jcl < p.cols_per_cta && km >= 0 && kp1 < p.n_rho &&
+                                           (unsigned)kp1 * pitch + 4u * cell_word_off<ACC16>(jcl) + 4 <= limit, HB_H4);
+                    const unsigned w0 = in ? *(const unsigned*)(colp + (size_t)km * p.pitch_b) : 0u;
+                    const unsigned w1 = in ? *(const unsigned*)(colp + (size_t)k * p.pitch_b) : 0u;
+                    const unsigned w2 = in ? *(const unsigned*)(colp + (size_t)kp1 * p.pitch_b) : 0u;
                     const unsigned msk = ACC16 ? 0xFFFFu : 0xFFFFFFFFu;
                     nb[dj + 1][0] = (vj && vkm) ? ((w0 >> sh) & msk) : 0u;
                     nb[dj + 1][1] = vj ? ((w1 >> sh) & msk) : 0u;
@@ -374,7 +399,8 @@ __global__ void __launch_bounds__(1024, 1) hough_event_kernel(const __grid_const
                 // strictly greater than the neighbours that precede in raster order, >= those that follow
                 const bool ok = a > nb[0][0] && a > nb[0][1] && a > nb[0][2] && a > nb[1][0] &&
                                 a >= nb[1][2] && a >= nb[2][0] && a >= nb[2][1] && a >= nb[2][2];
-                if (ok) red_shared_or((unsigned)__cvta_generic_to_shared(&pbm[jl * p.wpr + (k >> 5)]), 1u << (k & 31));
+                if (ok && HB_CHK(jl >= 0 && k >= 0 && 4 * (jl * p.wpr + (k >> 5)) + 4 <= p.pbm_bytes, HB_H4))
+                    red_shared_or((unsigned)__cvta_generic_to_shared(&pbm[jl * p.wpr + (k >> 5)]), 1u << (k & 31));
             };
             // Pass 1 streams the accumulator as uint4 and lists the VECTORS that hold a cell >= threshold (the list
             // lives in the part of the hit buffer without staged (u,v)); pass 2 gives every cell of a listed vector
@@ -388,6 +414,7 @@ __global__ void __launch_bounds__(1024, 1) hough_event_kernel(const __grid_const
             auto test_cell = [&](int v, int c) {
                 const int k = v / vpr, wv = v - k * vpr;
                 const int wi = 4 * wv + (ACC16 ? (c >> 1) : c);  // word index within the row
+                if (!HB_CHK(v >= 0 && k < p.n_rho && (unsigned)k * pitch + 4u * wi + 4 <= limit, HB_H4)) return;
                 const unsigned word = *(const unsigned*)(acc + (size_t)k * p.pitch_b + 4u * wi);
                 // u16: word G*32 + l holds columns 64G + l (low half) and 64G + 32 + l (high half); u32: word index IS the column
                 const int jl = ACC16 ? 64 * (wi >> 5) + (wi & 31) + 32 * (c & 1) : wi;
@@ -411,12 +438,16 @@ __global__ void __launch_bounds__(1024, 1) hough_event_kernel(const __grid_const
             auto scan_vec = [&](int v, const uint4& w) {
                 if (!vec_any(w)) return;
                 const int pos = atomicAdd(&misc[42], 1);
-                if (pos < vcap) { vlist[pos] = (unsigned)v; return; }
+                if (pos < vcap) {
+                    if (HB_CHK((single ? n : 0) * 8 + 4 * pos + 4 <= 8 * p.chunk, HB_H4)) vlist[pos] = (unsigned)v;
+                    return;
+                }
 #pragma unroll 1
                 for (int c = 0; c < CELLS; ++c) test_cell(v, c);
             };
             int v = tid;
             for (; v + 3 * nthreads < n_vec; v += 4 * nthreads) {   // four vectors per trip, one test
+                if (!HB_CHK(16u * (unsigned)(v + 3 * nthreads + 1) <= limit, HB_H4)) continue;
                 const uint4 w0 = acc4[v], w1 = acc4[v + nthreads], w2 = acc4[v + 2 * nthreads], w3 = acc4[v + 3 * nthreads];
                 bool any4;                                         // max over the 16 words: eight 3-input max, one compare
                 if (ACC16) {
@@ -437,10 +468,12 @@ __global__ void __launch_bounds__(1024, 1) hough_event_kernel(const __grid_const
                     scan_vec(v, w0); scan_vec(v + nthreads, w1); scan_vec(v + 2 * nthreads, w2); scan_vec(v + 3 * nthreads, w3);
                 }
             }
-            for (; v < n_vec; v += nthreads) scan_vec(v, acc4[v]);
+            for (; v < n_vec; v += nthreads)
+                if (HB_CHK(16u * (unsigned)(v + 1) <= limit, HB_H4)) scan_vec(v, acc4[v]);
             __syncthreads();
             const int n_items = min(misc[42], vcap) * CELLS;
-            for (int i = tid; i < n_items; i += nthreads) test_cell((int)vlist[i / CELLS], i % CELLS);
+            for (int i = tid; i < n_items; i += nthreads)
+                if (HB_CHK((single ? n : 0) * 8 + 4 * (i / CELLS) + 4 <= 8 * p.chunk, HB_H4)) test_cell((int)vlist[i / CELLS], i % CELLS);
         }
         __syncthreads();
 
@@ -449,7 +482,8 @@ __global__ void __launch_bounds__(1024, 1) hough_event_kernel(const __grid_const
         const int span = (W + nthreads - 1) / nthreads;
         const int w_lo = min(tid * span, W), w_hi = min(w_lo + span, W);
         int my_peaks = 0;
-        for (int w = w_lo; w < w_hi; ++w) my_peaks += __popc(pbm[w]);
+        for (int w = w_lo; w < w_hi; ++w)
+            if (HB_CHK(4 * w + 4 <= p.pbm_bytes, HB_H5)) my_peaks += __popc(pbm[w]);
         int cta_peaks;
         int pos = block_exscan(my_peaks, misc, cta_peaks);
         int base = 0, n_peaks = cta_peaks;
@@ -465,11 +499,12 @@ __global__ void __launch_bounds__(1024, 1) hough_event_kernel(const __grid_const
         }
         pos += base;
         for (int w = w_lo; w < w_hi && pos < p.max_peaks; ++w) {
-            unsigned bits = pbm[w];
+            unsigned bits = HB_CHK(4 * w + 4 <= p.pbm_bytes, HB_H5) ? pbm[w] : 0u;
             const int jl = w / p.wpr, kb = (w - jl * p.wpr) << 5;
             while (bits && pos < p.max_peaks) {
                 const int k = kb + __ffs(bits) - 1;
                 bits &= bits - 1;
+                if (!HB_CHK(jl < ncols && k < p.n_rho && pos >= 0, HB_H5)) continue;
                 hough_peak pk;
                 pk.theta_bin = (uint16_t)(col0 + jl);
                 pk.rho_bin = (uint16_t)k;
@@ -500,15 +535,18 @@ __global__ void __launch_bounds__(1024, 1) hough_event_kernel(const __grid_const
             const int w8_vec = (int)((cols_ub + 7) >> 3) * (p.w8_pitch >> 4);
             uint4* z = (uint4*)W8;
             const uint4 zz = make_uint4(0, 0, 0, 0);
-            for (int i = tid; i < w8_vec; i += nthreads) z[i] = zz;
-            for (int j = tid; j < p.n_theta; j += nthreads) colq[j] = 0;
+            for (int i = tid; i < w8_vec; i += nthreads)
+                if (HB_CHK(p.w8_off + 16 * (i + 1) <= p.mcf_off, HB_H6_SETUP)) z[i] = zz;
+            for (int j = tid; j < p.n_theta; j += nthreads)
+                if (HB_CHK(p.colq_off + 4 * (j + 1) <= p.region_bytes, HB_H6_SETUP)) colq[j] = 0;
             if (tid == 0) misc[41] = 0;
         }
         __syncthreads();
         for (int q = tid; q < n_stored; q += nthreads) {
             const hough_peak pk = p.peaks[(size_t)e * p.max_peaks + q];
             const int jlo = max(0, (int)pk.theta_bin - p.window), jhi = min(p.n_theta - 1, (int)pk.theta_bin + p.window);
-            for (int j = jlo; j <= jhi; ++j) colq[j] = 1;
+            for (int j = jlo; j <= jhi; ++j)
+                if (HB_CHK(j >= 0 && j < p.n_theta, HB_H6_SETUP)) colq[j] = 1;
         }
         __syncthreads();
         // number the marked columns (order irrelevant for the OR of S5)
@@ -521,15 +559,17 @@ __global__ void __launch_bounds__(1024, 1) hough_event_kernel(const __grid_const
             wbase = __shfl_sync(0xffffffffu, wbase, 0);
             if (any) {
                 const int q = wbase + __popc(bal & ((1u << lane) - 1u));
-                mcf[q] = p.cos_t[j];
-                msf[q] = p.sin_t[j];
-                colq[j] = q;
+                if (HB_CHK(q >= 0 && q < p.n_theta, HB_H6_SETUP)) {
+                    mcf[q] = p.cos_t[j];
+                    msf[q] = p.sin_t[j];
+                    colq[j] = q;
+                }
             }
         }
         __syncthreads();
         const int n_marked = misc[41];
         const int n_g8 = (n_marked + 7) >> 3;
-        if (tid < 8 * n_g8 - n_marked) {   // pad the last group with columns whose bits are never set
+        if (tid < 8 * n_g8 - n_marked && HB_CHK(n_marked + tid < p.n_theta + 8, HB_H6_SETUP)) {   // pad the last group with columns whose bits are never set
             mcf[n_marked + tid] = 0.0f;
             msf[n_marked + tid] = 0.0f;
         }
@@ -539,6 +579,7 @@ __global__ void __launch_bounds__(1024, 1) hough_event_kernel(const __grid_const
             const int klo = max(0, (int)pk.rho_bin - p.window), khi = min(p.n_rho - 1, (int)pk.rho_bin + p.window);
             for (int j = jlo; j <= jhi; ++j) {
                 const int cq = colq[j];
+                if (!HB_CHK(cq >= 0 && cq < n_marked && ((cq >> 3) + 1) * p.w8_pitch <= p.mcf_off - p.w8_off && (khi | 3) < p.w8_pitch, HB_H6_SETUP)) continue;
                 const unsigned bit4 = (1u << (cq & 7)) * 0x01010101u;
                 const unsigned row_s = (unsigned)__cvta_generic_to_shared(W8 + (cq >> 3) * p.w8_pitch);
                 for (int wd = klo >> 2; wd <= khi >> 2; ++wd) {
@@ -555,6 +596,7 @@ __global__ void __launch_bounds__(1024, 1) hough_event_kernel(const __grid_const
         auto keep_test = [&](float2 uv, bool valid) -> bool {
             unsigned hitbits = 0;
             for (int g8 = 0; g8 < n_g8; ++g8) {
+                if (!HB_CHK(8 * g8 + 8 <= p.n_theta + 8 && (g8 + 1) * p.w8_pitch <= p.mcf_off - p.w8_off && p.n_rho < p.w8_pitch, HB_KEEP)) break;
                 const float4 ca = *(const float4*)(mcf + 8 * g8), cb = *(const float4*)(mcf + 8 * g8 + 4);
                 const float4 sa = *(const float4*)(msf + 8 * g8), sb = *(const float4*)(msf + 8 * g8 + 4);
                 const unsigned char* row = W8 + g8 * p.w8_pitch;
@@ -583,7 +625,7 @@ __global__ void __launch_bounds__(1024, 1) hough_event_kernel(const __grid_const
                 const int ppos = block_exscan(kp ? 1 : 0, misc, blk_total);
                 if (valid) {
                     p.keep[beg + i] = kp ? 1 : 0;
-                    if (kp) {
+                    if (kp && HB_CHK(kept_base + ppos >= 0 && kept_base + ppos <= i, HB_H7)) {
                         if (p.kept_xy) p.kept_xy[beg + kept_base + ppos] = __ldg(&p.xy[beg + i]);
                         if (p.kept_idx) p.kept_idx[beg + kept_base + ppos] = i;
                     }
@@ -609,10 +651,10 @@ __global__ void __launch_bounds__(1024, 1) hough_event_kernel(const __grid_const
                     if (valid) uv = single ? hb[i] : conformal(__ldg(&p.xy[beg + i]), p.scale);
                     const bool kp = keep_test(uv, valid);
                     const unsigned bal = __ballot_sync(0xffffffffu, kp);
-                    if (lane == 0) stash[bl * nwarps + warp] = bal;
+                    if (lane == 0 && HB_CHK(bl < HOUGH_SEL_ROUND_BLOCKS, HB_H7)) stash[bl * nwarps + warp] = bal;
                     if (valid) p.keep[beg + i] = kp ? 1 : 0;
                     const int tot = __syncthreads_count(kp);
-                    if (tid == 0) cnt[bl] = tot;
+                    if (tid == 0 && HB_CHK(bl < HOUGH_SEL_ROUND_BLOCKS, HB_H7)) cnt[bl] = tot;
                 }
                 cg::this_cluster().sync();   // (D) counts of this round visible
                 // exclusive bases of the round's blocks (every CTA computes all; tiny)
@@ -621,7 +663,7 @@ __global__ void __launch_bounds__(1024, 1) hough_event_kernel(const __grid_const
                     for (int b = 0; b < rnb; b += 32) {
                         const int bb = b + lane;
                         int v = 0;
-                        if (bb < rnb) v = *(const int*)cg::this_cluster().map_shared_rank((void*)&cnt[bb / C], bb % C);
+                        if (bb < rnb && HB_CHK(bb / C < HOUGH_SEL_ROUND_BLOCKS, HB_H7)) v = *(const int*)cg::this_cluster().map_shared_rank((void*)&cnt[bb / C], bb % C);
                         int incl = v;
 #pragma unroll
                         for (int d = 1; d < 32; d <<= 1) {
@@ -641,6 +683,7 @@ __global__ void __launch_bounds__(1024, 1) hough_event_kernel(const __grid_const
                     if ((bal >> lane) & 1u) {
                         int ppos = gcnt[bb] + __popc(bal & ((1u << lane) - 1u));
                         for (int w2 = 0; w2 < warp; ++w2) ppos += __popc(stash[bl * nwarps + w2]);
+                        if (!HB_CHK(ppos >= 0 && ppos <= i && bb <= HOUGH_SEL_ROUND_BLOCKS * C, HB_H7)) continue;
                         if (p.kept_xy) p.kept_xy[beg + ppos] = __ldg(&p.xy[beg + i]);
                         if (p.kept_idx) p.kept_idx[beg + ppos] = i;
                     }
@@ -650,6 +693,13 @@ __global__ void __launch_bounds__(1024, 1) hough_event_kernel(const __grid_const
             }
             if (rank == 0 && tid == 0) p.counts[2 * e + 1] = kept_base;
         }
+#ifdef HOUGH_DEBUG_BOUNDS
+        {   // report skipped accesses: {HOUGH_DBG_SENTINEL, bit mask of the phases that violated}
+            if (CL) cg::this_cluster().sync();   // after rank 0's regular count writes
+            const int m = __syncthreads_or(dbg_viol ? (1 << dbg_viol) : 0);
+            if (m && tid == 0) { p.counts[2 * e] = HOUGH_DBG_SENTINEL; p.counts[2 * e + 1] = m; }
+        }
+#endif
     }
 }
 

@@ -1,15 +1,17 @@
-// microbench.cu -- measurement aids behind hough_bench_shared_atomics()
-// (include/hough.h).  They give the denominators of the vote roofline
-// (DESIGN.md "Roofline"): the SM's conflict-free shared-atomic rate and the
-// issue-slot bound of the voting loop's instruction mix.
+// microbench.cu -- measurement aids of include/hough_bench.h, built into libhough_bench.so (NOT into the
+// product library).  They give the denominator of the vote roofline (the SM's
+// conflict-free shared-atomic rate) and the issue cost of the voting loop's instruction classes.
+// Every shared-memory address formed here is either a compile-time layout offset or is masked / clamped
+// into the kernel's own allocation before use.
 #include <cstdio>
 
+#include "../../include/hough_bench.h"
 #include "hough_kernel.cuh"
 
 namespace {
 
-
-// variants 0-2: nothing but shared atomics.  8 atomics per loop trip.
+// ---------------------------------------------------------------- shared atomics alone
+// variants 0-2: nothing but shared atomics, address arithmetic in the loop.  8 atomics per loop trip.
 template <int VARIANT>
 __global__ void __launch_bounds__(1024, 1) atomics_kernel(long long iters, unsigned* sink) {
     extern __shared__ __align__(128) unsigned char smem[];
@@ -61,52 +63,69 @@ __global__ void __launch_bounds__(1024, 1) atomics_peak_kernel(long long iters, 
     if (sink && threadIdx.x == 0) sink[blockIdx.x] = a[threadIdx.x & 31];
 }
 
-// variants 3-4 and 6-8: the voting loop's instruction mix over a synthetic (u,v) buffer
-// (180 x 256 u16 geometry: 3 groups of 64 columns), with or without the atomics, scalar or packed
-// (fp32x2) arithmetic, row pitch 384 B (IMAD addressing) or 512 B (shift-add addressing).
-template <bool ATOMICS, bool PACKED, int PITCH>
-__global__ void __launch_bounds__(1024, 1) votemix_kernel(long long iters, unsigned* sink) {
+// ---------------------------------------------------------------- the voting loop, one instruction class at a time
+// MODE bits: 1 = atomics, 2 = clamp, 4 = IMAD row address (else IADD of the lane offset), 8 = packed fp32x2 (else scalar).
+// Geometry of the 180 x 256 u16 plan: 192 padded columns, 384-byte rows, 257 rows (the last one is the trash row).
+constexpr int VL_NRHO = 256, VL_PITCH = 384, VL_NHITS = 1024;
+constexpr int VL_SMEM = (VL_NRHO + 1) * VL_PITCH + VL_NHITS * 8;
+
+template <int MODE, int CPL>
+__global__ void __launch_bounds__(1024, 1) vote_loop_kernel(long long iters, unsigned* sink) {
     extern __shared__ __align__(128) unsigned char smem[];
-    const int N_RHO = 256, NHITS = 1024;
-    unsigned char* acc = smem;                               // (256 + 1 trash) rows
-    float2* hb = (float2*)(smem + (N_RHO + 1) * PITCH);      // 8 KB
-    for (int i = threadIdx.x; i < (N_RHO + 1) * PITCH / 4; i += blockDim.x) ((unsigned*)acc)[i] = 0;
-    for (int i = threadIdx.x; i < NHITS; i += blockDim.x) {
+    const unsigned pitch = VL_PITCH;
+    unsigned char* acc = smem;
+    float2* hb = (float2*)(smem + (VL_NRHO + 1) * VL_PITCH);
+    for (int i = threadIdx.x; i < (VL_NRHO + 1) * VL_PITCH / 4; i += blockDim.x) ((unsigned*)acc)[i] = 0;
+    for (int i = threadIdx.x; i < VL_NHITS; i += blockDim.x) {   // hits on the 48 layer radii: every bin is in range or clamped
         float r = 200.0f + 600.0f * (float)((i * 37) % 48) / 47.0f, phi = 0.0061359f * (float)i;
-        float x = r * cosf(phi), y = r * sinf(phi);
-        hb[i] = hough::conformal(make_float2(x, y), 1.0f);
+        hb[i] = hough::conformal(make_float2(r * cosf(phi), r * sinf(phi)), 1.0f);
     }
     __syncthreads();
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarps = blockDim.x >> 5;
-    const int g = warp % 3, stripe = warp / 3, n_stripes = nwarps / 3;
-    const int j0 = 64 * g + lane, j1 = j0 + 32;
-    const float th0 = 3.14159265f * j0 / 180.0f, th1 = 3.14159265f * j1 / 180.0f;
-    const float c0 = cosf(th0), c1 = cosf(th1), s0 = sinf(th0), s1 = sinf(th1);
+    constexpr int NG = 192 / (32 * CPL);
+    const int g = warp % NG, stripe = warp / NG, S = nwarps / NG;
+    hough::ull c2q[CPL / 2], s2q[CPL / 2];
+    float cq[CPL], sq[CPL];
+#pragma unroll
+    for (int q = 0; q < CPL; ++q) {
+        float th = 3.14159265f * (32 * (g * CPL + q) + lane) / 180.0f;
+        cq[q] = cosf(th);
+        sq[q] = sinf(th);
+    }
+#pragma unroll
+    for (int q = 0; q < CPL; q += 2) {
+        c2q[q / 2] = hough::pack2(cq[q], cq[q + 1]);
+        s2q[q / 2] = hough::pack2(sq[q], sq[q + 1]);
+    }
     const float rho_max = 1.0f / 334.0f, inv = 42752.0f;
-    const unsigned pitch = PITCH, limit = N_RHO * PITCH;
-    const unsigned lc0 = 4u * (g * 32 + lane) - HOUGH_MAGIC_BITS * pitch, lc1 = lc0;
-    const unsigned acc_s = (unsigned)__cvta_generic_to_shared(acc);
-    const unsigned trash = limit + 4u * (g * 32 + lane);
-    const hough::ull C2 = hough::pack2(c0, c1), S2 = hough::pack2(s0, s1);
+    const unsigned wbase = g * (CPL / 2) * 128 + 4 * lane;
+    const unsigned lc0 = wbase - HOUGH_MAGIC_BITS * pitch, trash0 = VL_NRHO * pitch + wbase;
     unsigned chk = 0;
-    if (stripe < n_stripes) {
+    if (stripe < S) {
         for (long long it = 0; it < iters; ++it) {
-#pragma unroll 4
-            for (int i = stripe; i < NHITS; i += n_stripes) {
+#pragma unroll 2
+            for (int i = stripe; i < VL_NHITS; i += S) {
                 const float2 uv = hb[i];
-                unsigned b0, b1;
-                if (PACKED) {
-                    hough::bin_bits2(uv.x, uv.y, C2, S2, rho_max, inv, b0, b1);
-                } else {
-                    b0 = hough::bin_bits(uv.x, uv.y, c0, s0, rho_max, inv);
-                    b1 = hough::bin_bits(uv.x, uv.y, c1, s1, rho_max, inv);
-                }
-                const unsigned rel0 = b0 * pitch + lc0, rel1 = b1 * pitch + lc1;
-                if (ATOMICS) {
-                    hough::vote_add(acc_s + min(rel0, trash), 1u);
-                    hough::vote_add(acc_s + min(rel1, trash), 0x10000u);
-                } else {
-                    chk += (rel0 < limit ? rel0 : 0u) ^ (rel1 < limit ? rel1 : 0u);
+#pragma unroll
+                for (int q = 0; q < CPL; q += 2) {
+                    unsigned b0, b1;
+                    if (MODE & 8) {
+                        hough::bin_bits2(uv.x, uv.y, c2q[q / 2], s2q[q / 2], rho_max, inv, b0, b1);
+                    } else {
+                        b0 = hough::bin_bits(uv.x, uv.y, cq[q], sq[q], rho_max, inv);
+                        b1 = hough::bin_bits(uv.x, uv.y, cq[q + 1], sq[q + 1], rho_max, inv);
+                    }
+                    unsigned r0, r1;
+                    if (MODE & 4) { r0 = b0 * pitch + lc0; r1 = b1 * pitch + lc0; }
+                    else { r0 = b0 + lc0; r1 = b1 + lc0; }
+                    if (MODE & 2) { r0 = min(r0, trash0); r1 = min(r1, trash0); }
+                    else { r0 &= 0xFFFCu; r1 &= 0xFFFCu; }             // stays inside the accumulator without a clamp
+                    if (MODE & 1) {
+                        atomicAdd((unsigned*)(acc + r0 + 128 * (q / 2)), 1u);
+                        atomicAdd((unsigned*)(acc + r1 + 128 * (q / 2)), 0x10000u);
+                    } else {
+                        chk += r0 ^ r1;
+                    }
                 }
             }
         }
@@ -115,53 +134,158 @@ __global__ void __launch_bounds__(1024, 1) votemix_kernel(long long iters, unsig
     if (sink && (chk == 0x12345u || threadIdx.x == 0)) sink[blockIdx.x] = ((unsigned*)acc)[lane] + chk;
 }
 
-}  // namespace
+// ---------------------------------------------------------------- one instruction class at a time
+// 32 instructions per loop trip over 16 independent registers (two rounds), inline PTX so that nothing folds.
+#define ISSUE_R16(OP)                                                                                         \
+    OP(0) OP(1) OP(2) OP(3) OP(4) OP(5) OP(6) OP(7) OP(8) OP(9) OP(10) OP(11) OP(12) OP(13) OP(14) OP(15)
+#define OP_FMUL(i) asm volatile("mul.rn.f32 %0, %0, %1;" : "+f"(f[i]) : "f"(fc));
+#define OP_FADD(i) asm volatile("add.rn.f32 %0, %0, %1;" : "+f"(f[i]) : "f"(fc));
+#define OP_FFMA(i) asm volatile("fma.rn.f32 %0, %0, %1, %2;" : "+f"(f[i]) : "f"(fc), "f"(fd));
+#define OP_FMUL2(i) asm volatile("mul.rn.f32x2 %0, %0, %1;" : "+l"(d[i]) : "l"(dc));
+#define OP_FADD2(i) asm volatile("add.rn.f32x2 %0, %0, %1;" : "+l"(d[i]) : "l"(dc));
+#define OP_IMAD(i) asm volatile("mad.lo.u32 %0, %0, %1, %2;" : "+r"(u[i]) : "r"(uc), "r"(ud));
+#define OP_MIN(i) asm volatile("min.u32 %0, %0, %1;" : "+r"(u[i]) : "r"(u[(i + 5) & 15]));
+#define OP_IADD(i) asm volatile("add.u32 %0, %0, %1;" : "+r"(u[i]) : "r"(u[(i + 5) & 15]));
+#define OP_LOP3(i) asm volatile("lop3.b32 %0, %0, %1, %2, 0x96;" : "+r"(u[i]) : "r"(uc), "r"(u[(i + 5) & 15]));
+#define OP_LEA(i) asm volatile("{ .reg .u32 t; shl.b32 t, %0, 7; add.u32 %0, t, %1; }" : "+r"(u[i]) : "r"(uc));
+#define OP_FMUL_MIN(i) OP_FMUL(i) OP_MIN(i)
+#define OP_FMUL_IMAD(i) OP_FMUL(i) OP_IMAD(i)
+#define OP_FMUL2_MIN(i) OP_FMUL2(i) OP_MIN(i)
+#define OP_FMUL_IADD(i) OP_FMUL(i) OP_IADD(i)
 
-extern "C" int hough_bench_shared_atomics(int variant, int ctas_per_sm, int threads, long long iters, double* out_rate) {
-    if (variant < 0 || variant > 8 || ctas_per_sm < 1 || threads < 32 || threads > 1024 || (threads & 31) || iters < 1 || !out_rate)
-        return HOUGH_ERR_INVALID_ARG;
-    int dev = 0, sms = 0;
-    if (cudaGetDevice(&dev) != cudaSuccess) return HOUGH_ERR_CUDA;
-    if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) return HOUGH_ERR_CUDA;
-    const int grid = sms * ctas_per_sm;
-    unsigned* sink = nullptr;
-    if (cudaMalloc(&sink, sizeof(unsigned) * grid) != cudaSuccess) return HOUGH_ERR_NOMEM;
-    size_t smem = (variant <= 2 || variant == 5) ? 32768 : (257 * (variant == 8 ? 512 : 384) + 8192);
-    const void* fn = nullptr;
-    switch (variant) {
-        case 0: fn = (const void*)&atomics_kernel<0>; break;
-        case 1: fn = (const void*)&atomics_kernel<1>; break;
-        case 2: fn = (const void*)&atomics_kernel<2>; break;
-        case 3: fn = (const void*)&votemix_kernel<false, false, 384>; break;
-        case 4: fn = (const void*)&votemix_kernel<true, false, 384>; break;
-        case 6: fn = (const void*)&votemix_kernel<false, true, 384>; break;
-        case 7: fn = (const void*)&votemix_kernel<true, true, 384>; break;
-        case 8: fn = (const void*)&votemix_kernel<true, true, 512>; break;
-        default: fn = (const void*)&atomics_peak_kernel; break;
+template <int KIND>
+__global__ void __launch_bounds__(1024, 1) issue_kernel(long long iters, unsigned* sink, float fseed, unsigned useed) {
+    float f[16];
+    hough::ull d[16];
+    unsigned u[16];
+#pragma unroll
+    for (int i = 0; i < 16; ++i) {
+        f[i] = fseed + (float)(threadIdx.x + i);
+        d[i] = hough::pack2(f[i], f[i] + 0.5f);
+        u[i] = useed * (threadIdx.x + 7u * i + 1u);
     }
-    cudaError_t e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    const float fc = 1.0f + fseed * 1e-7f, fd = fseed * 1e-9f;
+    const hough::ull dc = hough::pack2(fc, fc);
+    const unsigned uc = useed | 3u, ud = useed + 11u;
+    for (long long it = 0; it < iters; ++it) {
+        if (KIND == 0) { ISSUE_R16(OP_FMUL) ISSUE_R16(OP_FMUL) }
+        if (KIND == 1) { ISSUE_R16(OP_FADD) ISSUE_R16(OP_FADD) }
+        if (KIND == 2) { ISSUE_R16(OP_FFMA) ISSUE_R16(OP_FFMA) }
+        if (KIND == 3) { ISSUE_R16(OP_FMUL2) ISSUE_R16(OP_FMUL2) }
+        if (KIND == 4) { ISSUE_R16(OP_FADD2) ISSUE_R16(OP_FADD2) }
+        if (KIND == 5) { ISSUE_R16(OP_IMAD) ISSUE_R16(OP_IMAD) }
+        if (KIND == 6) { ISSUE_R16(OP_MIN) ISSUE_R16(OP_MIN) }
+        if (KIND == 7) { ISSUE_R16(OP_IADD) ISSUE_R16(OP_IADD) }
+        if (KIND == 8) { ISSUE_R16(OP_LOP3) ISSUE_R16(OP_LOP3) }
+        if (KIND == 9) { ISSUE_R16(OP_LEA) ISSUE_R16(OP_LEA) }
+        if (KIND == 10) { ISSUE_R16(OP_FMUL_MIN) }
+        if (KIND == 11) { ISSUE_R16(OP_FMUL_IMAD) }
+        if (KIND == 12) { ISSUE_R16(OP_FMUL2_MIN) }
+        if (KIND == 13) { ISSUE_R16(OP_FMUL_IADD) }
+    }
+    constexpr bool USES_F = KIND <= 2 || KIND == 10 || KIND == 11 || KIND == 13, USES_D = KIND == 3 || KIND == 4 || KIND == 12,
+                   USES_U = KIND >= 5 && KIND != 12 || KIND == 12;
+    unsigned acc = 0;
+#pragma unroll
+    for (int i = 0; i < 16; ++i) {   // only the registers this kind works on stay live
+        if (USES_F) acc ^= __float_as_uint(f[i]);
+        if (USES_D) acc ^= (unsigned)d[i] ^ (unsigned)(d[i] >> 32);
+        if (USES_U) acc ^= u[i];
+    }
+    if (sink && (acc == 0x12345u || threadIdx.x == 0)) sink[blockIdx.x] = acc;
+}
+
+// ---------------------------------------------------------------- host side
+int time_kernel(const void* fn, int grid, int threads, size_t smem, void** args, float* ms_out) {
+    if (smem > 48 * 1024 && cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return -3;
     cudaEvent_t ev0, ev1;
-    cudaEventCreate(&ev0); cudaEventCreate(&ev1);
-    void* args[2] = {(void*)&iters, (void*)&sink};
-    float ms = 0.0f;
+    if (cudaEventCreate(&ev0) != cudaSuccess || cudaEventCreate(&ev1) != cudaSuccess) return -3;
+    cudaError_t e = cudaSuccess;
     for (int rep = 0; rep < 3 && e == cudaSuccess; ++rep) {   // 2 warm-ups, the third is timed
         if (rep == 2) cudaEventRecord(ev0, 0);
         e = cudaLaunchKernel(fn, dim3(grid), dim3(threads), args, smem, 0);
         if (rep == 2) cudaEventRecord(ev1, 0);
     }
     if (e == cudaSuccess) e = cudaDeviceSynchronize();
-    if (e == cudaSuccess) cudaEventElapsedTime(&ms, ev0, ev1);
-    cudaEventDestroy(ev0); cudaEventDestroy(ev1);
+    if (e == cudaSuccess) e = cudaEventElapsedTime(ms_out, ev0, ev1);
+    cudaEventDestroy(ev0);
+    cudaEventDestroy(ev1);
+    return e == cudaSuccess ? 0 : -3;
+}
+
+int device_grid(int ctas_per_sm, int* grid) {
+    int dev = 0, sms = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) return -3;
+    if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) return -3;
+    *grid = sms * ctas_per_sm;
+    return 0;
+}
+
+bool bad_shape(int ctas_per_sm, int threads, long long iters, const double* out) {
+    return ctas_per_sm < 1 || ctas_per_sm > 8 || threads < 32 || threads > 1024 || (threads & 31) || iters < 1 || !out;
+}
+
+}  // namespace
+
+extern "C" int hough_bench_shared_atomics(int variant, int ctas_per_sm, int threads, long long iters, double* out_rate) {
+    if ((variant != 0 && variant != 1 && variant != 2 && variant != 5) || bad_shape(ctas_per_sm, threads, iters, out_rate)) return -1;
+    int grid = 0;
+    if (int rc = device_grid(ctas_per_sm, &grid)) return rc;
+    unsigned* sink = nullptr;
+    if (cudaMalloc(&sink, sizeof(unsigned) * grid) != cudaSuccess) return -4;
+    const void* fn = variant == 0 ? (const void*)&atomics_kernel<0> : variant == 1 ? (const void*)&atomics_kernel<1>
+                   : variant == 2 ? (const void*)&atomics_kernel<2> : (const void*)&atomics_peak_kernel;
+    void* args[2] = {(void*)&iters, (void*)&sink};
+    float ms = 0.0f;
+    const int rc = time_kernel(fn, grid, threads, 32768, args, &ms);
     cudaFree(sink);
-    if (e != cudaSuccess) return HOUGH_ERR_CUDA;
-    double per_thread = (variant <= 2 || variant == 5) ? 8.0 * (double)iters : 0.0;
-    double total;
-    if (variant <= 2 || variant == 5) {
-        total = per_thread * (double)threads * (double)grid;
-    } else {
-        const int nwarps = threads / 32, n_stripes = nwarps / 3;
-        total = (double)iters * 1024.0 * 192.0 * (double)grid * (n_stripes > 0 ? 1.0 : 0.0);   // lane-votes incl. padded lanes
+    if (rc) return rc;
+    *out_rate = 8.0 * (double)iters * (double)threads * (double)grid / ((double)ms * 1e-3);
+    return 0;
+}
+
+extern "C" int hough_bench_vote_loop(int mode, int cpl, int ctas_per_sm, int threads, long long iters, double* out_rate) {
+    if (mode < 0 || mode > 15 || (cpl != 2 && cpl != 6) || bad_shape(ctas_per_sm, threads, iters, out_rate)) return -1;
+    if ((threads / 32) < 192 / (32 * cpl)) return -1;
+    int grid = 0;
+    if (int rc = device_grid(ctas_per_sm, &grid)) return rc;
+    const void* fn = nullptr;
+#define VL_CASE(M) case M: fn = cpl == 6 ? (const void*)&vote_loop_kernel<M, 6> : (const void*)&vote_loop_kernel<M, 2>; break;
+    switch (mode) {
+        VL_CASE(0) VL_CASE(1) VL_CASE(2) VL_CASE(3) VL_CASE(4) VL_CASE(5) VL_CASE(6) VL_CASE(7)
+        VL_CASE(8) VL_CASE(9) VL_CASE(10) VL_CASE(11) VL_CASE(12) VL_CASE(13) VL_CASE(14) VL_CASE(15)
     }
-    *out_rate = total / ((double)ms * 1e-3);
-    return HOUGH_OK;
+#undef VL_CASE
+    unsigned* sink = nullptr;
+    if (cudaMalloc(&sink, sizeof(unsigned) * grid) != cudaSuccess) return -4;
+    void* args[2] = {(void*)&iters, (void*)&sink};
+    float ms = 0.0f;
+    const int rc = time_kernel(fn, grid, threads, VL_SMEM, args, &ms);
+    cudaFree(sink);
+    if (rc) return rc;
+    const int ng = 192 / (32 * cpl), stripes = (threads / 32) / ng;
+    *out_rate = (stripes > 0 ? 1.0 : 0.0) * (double)iters * (double)VL_NHITS * 192.0 * (double)grid / ((double)ms * 1e-3);
+    return 0;
+}
+
+extern "C" int hough_bench_issue_rate(int kind, int ctas_per_sm, int threads, long long iters, double* out_rate) {
+    if (kind < 0 || kind > 13 || bad_shape(ctas_per_sm, threads, iters, out_rate)) return -1;
+    int grid = 0;
+    if (int rc = device_grid(ctas_per_sm, &grid)) return rc;
+    const void* fns[14] = {
+        (const void*)&issue_kernel<0>, (const void*)&issue_kernel<1>, (const void*)&issue_kernel<2>, (const void*)&issue_kernel<3>,
+        (const void*)&issue_kernel<4>, (const void*)&issue_kernel<5>, (const void*)&issue_kernel<6>, (const void*)&issue_kernel<7>,
+        (const void*)&issue_kernel<8>, (const void*)&issue_kernel<9>, (const void*)&issue_kernel<10>, (const void*)&issue_kernel<11>,
+        (const void*)&issue_kernel<12>, (const void*)&issue_kernel<13>};
+    unsigned* sink = nullptr;
+    if (cudaMalloc(&sink, sizeof(unsigned) * grid) != cudaSuccess) return -4;
+    float fseed = 1.0f;
+    unsigned useed = 0x9E3779B1u;
+    void* args[4] = {(void*)&iters, (void*)&sink, (void*)&fseed, (void*)&useed};
+    float ms = 0.0f;
+    const int rc = time_kernel(fns[kind], grid, threads, 0, args, &ms);
+    cudaFree(sink);
+    if (rc) return rc;
+    *out_rate = 32.0 * (double)iters * (double)(threads / 32) * (double)grid / ((double)ms * 1e-3);   // warp-instructions/s
+    return 0;
 }

@@ -162,12 +162,74 @@ def test_cfg4_sweep_sampled_parity_100k(hb):
 
 
 # ---------------------------------------------------------------- variants of the launch
-@pytest.mark.parametrize("cluster", [2, 4])
+@pytest.mark.parametrize("cluster", [2, 4, 8])
 def test_forced_cluster_matches_oracle(hb, cluster):
     w = si.config(1)
     xy, off, _ = si.generate(w, 40)
     g, _ = run_both(hb, w, xy, off, cluster_size=cluster)
     assert g["info"]["CLUSTER_SIZE"] == cluster
+
+
+def test_cluster_grid_360x512_u32_plans_eight_ctas(hb):
+    # 720 KB of u32 cells: 90 columns per CTA pad to 128 (262 KB, too much), so the planner takes 8 CTAs of 45 columns
+    w = si.config(5)
+    xy, off, _ = si.generate(w, 16)
+    g, _ = run_both(hb, w, xy, off, acc_dtype="u32")
+    assert g["info"]["CLUSTER_SIZE"] == 8 and g["info"]["ACC_BITS"] == 32
+
+
+@pytest.mark.parametrize("cluster", [2, 8])
+def test_cluster_with_degenerate_hits_takes_the_slow_path(hb, cluster):
+    w = si.config(0)
+    xy, off, _ = si.generate(w, 3)
+    bad = np.array([[0, 0], [np.inf, 1], [1e-3, 0], [0, -1e-3], [1e-20, 1e-20], [np.nan, 5], [1e-30, 0],
+                    [1e30, 1e30], [-1e-3, 1e-3], [3e38, 0]], dtype=np.float32)
+    xy2 = np.concatenate([xy[:off[1]], bad, xy[off[1]:]])
+    off2 = off.copy()
+    off2[1:] += len(bad)
+    g, o = run_both(hb, w, xy2, off2, threshold=5, cluster_size=cluster)
+    assert o.accum[0].sum() > 0
+    run_both(hb, w, xy2, off2, threshold=5, cluster_size=cluster, vote_path=1)
+
+
+@pytest.mark.parametrize("cluster,acc", [(2, "u16"), (4, "u32")])
+def test_cluster_with_an_event_larger_than_the_staging_chunk(hb, cluster, acc):
+    w = si.config(3)
+    xy, off, _ = si.generate(w, 6)
+    big = np.ascontiguousarray(xy[:off[6]])             # ~17000 hits as ONE event: staged in several chunks
+    off_big = np.array([0, len(big)], dtype=np.int32)
+    g, _ = run_both(hb, w, big, off_big, threshold=60, cluster_size=cluster, acc_dtype=acc)
+    assert g["info"]["CHUNK_HITS"] < len(big) and g["info"]["CLUSTER_SIZE"] == cluster
+
+
+@pytest.mark.parametrize("max_peaks", [0, 1, 3])
+def test_cluster_with_max_peaks_truncation(hb, max_peaks):
+    w = si.config(2)
+    xy, off, _ = si.generate(w, 8)
+    g, o = run_both(hb, w, xy, off, max_peaks=max_peaks, cluster_size=2)
+    assert o.counts[:, 0].max() > 64 and g["info"]["CLUSTER_SIZE"] == 2
+
+
+@pytest.mark.parametrize("cluster,window", [(2, 2), (4, 0), (8, 3)])
+def test_cluster_with_windows(hb, cluster, window):
+    w = si.config(1)
+    xy, off, _ = si.generate(w, 12)
+    run_both(hb, w, xy, off, window=window, cluster_size=cluster)
+
+
+def test_cluster_selection_runs_a_second_round(hb):
+    # more than HOUGH_SEL_ROUND_BLOCKS (32) x C x threads hits in one u32 event: the clustered selection's round loop iterates
+    rng = np.random.default_rng(8)
+    n = 32 * 2 * 1024 + 5000
+    r = 200.0 + rng.integers(0, 48, n) * (600.0 / 47.0)
+    phi = rng.uniform(0, 2 * np.pi, n)
+    xy = np.stack([r * np.cos(phi), r * np.sin(phi)], axis=1).astype(np.float32)
+    w = si.config(1)
+    xy1, off1, _ = si.generate(w, 2)
+    xy = np.concatenate([xy1[:off1[1]], xy, xy1[off1[1]:]])
+    off = np.array([0, off1[1], off1[1] + n, off1[2] + n], dtype=np.int32)
+    g, o = run_both(hb, w, xy, off, acc_dtype="u32", cluster_size=2, threshold=500, window=1, max_peaks=256, accum=False)
+    assert g["info"]["THREADS"] * 32 * 2 < n and 0 < o.counts[1, 1] < n
 
 
 def test_one_cta_per_sm_and_slow_vote_path(hb):
@@ -343,3 +405,105 @@ def test_default_trig_table_equals_harness_table(hb):
 def test_shared_atomic_microbench_runs(hb):
     r = hb.hough_bench_shared_atomics(0, 2, 512, 2000)
     assert r > 1e11
+
+
+def test_two_live_handles_with_different_grids_interleave(hb):
+    # the dynamic-shared-memory attribute belongs to the kernel, not the handle: a second, smaller handle of the same
+    # instantiation must not break the first
+    import torch
+    w1, w0 = si.config(1), si.config(0)                # 180 x 256 and 180 x 128, both u16 with the same template arguments
+    xy1, off1, _ = si.generate(w1, 20)
+    xy0, off0, _ = si.generate(w0, 8)
+    t1, t0 = si.trig_table(w1.n_theta), si.trig_table(w0.n_theta)
+    h1 = hb.Hough(w1.n_theta, w1.n_rho, w1.rho_max, w1.threshold, w1.window, trig_table=t1)
+    h0 = hb.Hough(w0.n_theta, w0.n_rho, w0.rho_max, w0.threshold, w0.window, trig_table=t0)   # created AFTER h1, smaller
+    assert h0.info(hb.HOUGH_INFO_SMEM_BYTES) < h1.info(hb.HOUGH_INFO_SMEM_BYTES)
+    o1 = oracle.run(xy1, off1, w1.n_theta, w1.n_rho, w1.rho_max, w1.threshold, w1.window, t1[0], t1[1])
+    o0 = oracle.run(xy0, off0, w0.n_theta, w0.n_rho, w0.rho_max, w0.threshold, w0.window, t0[0], t0[1])
+    d1 = (torch.from_numpy(xy1).cuda(), torch.from_numpy(off1).cuda())
+    d0 = (torch.from_numpy(xy0).cuda(), torch.from_numpy(off0).cuda())
+    for _ in range(3):
+        a = h1.run(*d1)
+        b = h0.run(*d0)
+        torch.cuda.synchronize()
+        assert np.array_equal(a["counts"].cpu().numpy(), o1.counts) and np.array_equal(a["keep"].cpu().numpy(), o1.keep)
+        assert np.array_equal(b["counts"].cpu().numpy(), o0.counts) and np.array_equal(b["keep"].cpu().numpy(), o0.keep)
+    h1.close()
+    h0.close()
+
+
+def test_cuda_graph_capture_and_replay(hb):
+    # include/hough.h promises that hough_run can be captured: it never synchronises, allocates or reads device data
+    import torch
+    w = si.config(1)
+    xy, off, _ = si.generate(w, 50)
+    table = si.trig_table(w.n_theta)
+    o = oracle.run(xy, off, w.n_theta, w.n_rho, w.rho_max, w.threshold, w.window, table[0], table[1], max_peaks=w.max_peaks)
+    h = hb.Hough(w.n_theta, w.n_rho, w.rho_max, w.threshold, w.window, trig_table=table)
+    d_xy, d_off = torch.from_numpy(xy).cuda(), torch.from_numpy(off).cuda()
+    out = h.alloc_outputs(len(xy), 50)
+    s = torch.cuda.Stream()
+    s.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(s):
+        h.run(d_xy, d_off, out=out, stream=s)            # warm-up outside the capture
+    torch.cuda.synchronize()
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(graph, stream=s):
+        h.run(d_xy, d_off, out=out, stream=torch.cuda.current_stream())
+    for rep in range(3):
+        for v in out.values():
+            v.fill_(-1 if v.dtype != torch.uint8 else 9)
+        graph.replay()
+        torch.cuda.synchronize()
+        assert np.array_equal(out["counts"].cpu().numpy(), o.counts), rep
+        assert np.array_equal(out["keep"].cpu().numpy(), o.keep), rep
+        p3 = hb.unpack_peaks(out["peaks"])
+        for e in range(50):
+            ns = min(int(o.counts[e, 0]), w.max_peaks)
+            assert np.array_equal(p3[e, :ns], o.peaks[e, :ns])
+    h.close()
+
+
+def test_marshalling_rejects_wrong_dtype_device_and_length(hb):
+    import torch
+    w = si.config(0)
+    xy, off, _ = si.generate(w, 4)
+    h = hb.Hough(w.n_theta, w.n_rho, w.rho_max, w.threshold, w.window)
+    d_xy, d_off = torch.from_numpy(xy).cuda(), torch.from_numpy(off).cuda()
+    out = h.alloc_outputs(len(xy), 4)
+    ok = (d_xy, d_off, 4, out["keep"], out["peaks"], out["counts"])
+    hb.hough_run(h.ctx, *ok)
+    for bad in ((d_xy, d_off.long(), 4, out["keep"], out["peaks"], out["counts"]),            # int64 offsets
+                (d_xy.cpu(), d_off, 4, out["keep"], out["peaks"], out["counts"]),             # host tensor
+                (d_xy, d_off, 4, out["keep"][: len(xy) // 2], out["peaks"], out["counts"]),    # keep mask too short
+                (d_xy.double(), d_off, 4, out["keep"], out["peaks"], out["counts"]),
+                (d_xy, d_off, 4, out["keep"], out["peaks"][:2], out["counts"]),               # peaks too short
+                (d_xy.t().contiguous().t(), d_off, 4, out["keep"], out["peaks"], out["counts"])):  # not contiguous
+        with pytest.raises(hb.HoughError):
+            hb.hough_run(h.ctx, *bad)
+    torch.cuda.synchronize()
+    h.close()
+
+
+def test_second_device_when_present(hb):
+    import torch
+    if torch.cuda.device_count() < 2:
+        pytest.skip("one GPU")
+    w = si.config(0)
+    xy, off, _ = si.generate(w, 4)
+    table = si.trig_table(w.n_theta)
+    o = oracle.run(xy, off, w.n_theta, w.n_rho, w.rho_max, w.threshold, w.window, table[0], table[1])
+    with torch.cuda.device(1):
+        h = hb.Hough(w.n_theta, w.n_rho, w.rho_max, w.threshold, w.window, trig_table=table)
+        out = h.run(torch.from_numpy(xy).cuda(), torch.from_numpy(off).cuda())
+        torch.cuda.synchronize()
+        assert np.array_equal(out["counts"].cpu().numpy(), o.counts)
+    with pytest.raises(hb.HoughError):                   # the handle belongs to device 1; device 0 is current
+        h.run(torch.from_numpy(xy).cuda(), torch.from_numpy(off).cuda())
+    h.close()
+
+
+def test_measurement_aids_run(hb):
+    assert hb.hough_bench_shared_atomics(5, 1, 1024, 500) > 1e12
+    assert hb.hough_bench_vote_loop(15, 6, 2, 512, 2) > 1e11
+    assert hb.hough_bench_issue_rate(0, 1, 512, 200) > 1e10

@@ -22,9 +22,17 @@
 // Row n_rho is a trash row (one full pitch) that swallows the out-of-range votes and those of the padding columns.
 // In the vote phase a warp owns a group of 32*CPL adjacent columns (CPL = 2, 4 or 6 per lane) and a
 // stripe of the hits: one broadcast LDS.64 of (u,v) feeds CPL votes per lane.
+//
+// HOUGH_HOST_EMU (tests/simt_emu only): the same source is compiled by g++ against a SIMT shim (fibers, barriers, warp
+// collectives, a per-CTA shared-memory buffer) so that the CPU tests can execute the kernel's LOGIC -- indexing, phase
+// order, bounds -- against the oracle without a GPU.  The shim supplies the CUDA names; only the inline PTX below has
+// a host restatement.  It is test infrastructure: nothing in the product path is built with it.
 #pragma once
+#ifndef HOUGH_HOST_EMU
 #include <cooperative_groups.h>
 #include <cuda_runtime.h>
+#define HOUGH_DYN_SMEM(name) extern __shared__ __align__(128) unsigned char name[]
+#endif
 #include <stdint.h>
 
 #include "../../include/hough.h"
@@ -93,6 +101,11 @@ struct KParams {
 };
 
 // ---------------------------------------------------------------- small helpers
+#ifdef HOUGH_HOST_EMU
+inline void red_shared_add(unsigned saddr, unsigned v) { *(unsigned*)emu::shared_ptr(saddr) += v; }
+inline void vote_add(unsigned saddr, unsigned v) { *(unsigned*)emu::shared_ptr(saddr) += v; }
+inline void red_shared_or(unsigned saddr, unsigned v) { *(unsigned*)emu::shared_ptr(saddr) |= v; }
+#else
 __device__ __forceinline__ void red_shared_add(unsigned saddr, unsigned v) {
     asm volatile("red.shared.add.u32 [%0], %1;" ::"r"(saddr), "r"(v) : "memory");
 }
@@ -105,6 +118,7 @@ __device__ __forceinline__ void vote_add(unsigned saddr, unsigned v) {
 __device__ __forceinline__ void red_shared_or(unsigned saddr, unsigned v) {
     asm volatile("red.shared.or.b32 [%0], %1;" ::"r"(saddr), "r"(v) : "memory");
 }
+#endif
 
 // S1: d = fl(fl(x*x)+fl(y*y)); u = scale*fl(x/d); v = scale*fl(y/d).  Eq. (1).
 __device__ __forceinline__ float2 conformal(float2 h, float scale) {
@@ -132,6 +146,22 @@ __device__ __forceinline__ unsigned bin_bits(float u, float v, float c, float s,
 // even under --fmad=false), and it cannot do so when the flush modes differ.  The flush itself never
 // acts: the fast path only takes hits whose products with every non-zero table entry are normal
 // (KParams::ftz_min); build.py rejects any FFMA2 in the SASS.
+#ifdef HOUGH_HOST_EMU
+inline ull pack2(float lo, float hi) { return (ull)__float_as_uint(lo) | ((ull)__float_as_uint(hi) << 32); }
+// host restatement of the packed sequence, lane by lane, INCLUDING the flush-to-zero of the two products' inputs and
+// results, so that a non-tame hit on the fast path would show up as a mismatch against the oracle
+inline void bin_bits2(float u, float v, ull c2, ull s2, float rho_max, float inv, unsigned& b0, unsigned& b1) {
+    unsigned out[2];
+    for (int h = 0; h < 2; ++h) {
+        const float c = __uint_as_float((unsigned)(c2 >> (32 * h))), s = __uint_as_float((unsigned)(s2 >> (32 * h)));
+        const float p1 = emu::ftz(__fmul_rn(emu::ftz(u), emu::ftz(c))), p2 = emu::ftz(__fmul_rn(emu::ftz(v), emu::ftz(s)));
+        const float t = __fmul_rn(__fadd_rn(__fadd_rn(p1, p2), rho_max), inv);
+        out[h] = __float_as_uint(__fadd_rd(t, HOUGH_MAGIC_F));
+    }
+    b0 = out[0];
+    b1 = out[1];
+}
+#else
 __device__ __forceinline__ ull pack2(float lo, float hi) {
     ull r;
     asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
@@ -149,6 +179,7 @@ __device__ __forceinline__ void bin_bits2(float u, float v, ull c2, ull s2, floa
     asm("add.rm.f32x2 %0, %1, %2;" : "=l"(y) : "l"(t), "l"(mg2));
     asm("mov.b64 {%0, %1}, %2;" : "=r"(b0), "=r"(b1) : "l"(y));
 }
+#endif
 
 // S2, scalar and literal (the slow exact path and the reference for the trick).  Returns k or -1.
 __device__ __forceinline__ int bin_exact(float u, float v, float c, float s, float rho_max, float inv, int n_rho) {
@@ -203,7 +234,7 @@ __device__ __forceinline__ unsigned cell_from(const unsigned char* acc, int pitc
 // ---------------------------------------------------------------- the kernel
 template <bool ACC16, bool CL, int CPL>
 __global__ void __launch_bounds__(1024, 1) hough_event_kernel(const __grid_constant__ KParams p) {
-    extern __shared__ __align__(128) unsigned char smem[];
+    HOUGH_DYN_SMEM(smem);
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int nthreads = blockDim.x, nwarps = nthreads >> 5;
 
@@ -212,8 +243,13 @@ __global__ void __launch_bounds__(1024, 1) hough_event_kernel(const __grid_const
     const int C = p.csize;
     int cluster_id = blockIdx.x, n_clusters = gridDim.x;
     if (CL) {   // the hardware's own cluster index: no division by the run-time cluster size
+#ifdef HOUGH_HOST_EMU
+        cluster_id = emu::cluster_id();
+        n_clusters = emu::n_clusters();
+#else
         asm("mov.u32 %0, %%clusterid.x;" : "=r"(cluster_id));
         asm("mov.u32 %0, %%nclusterid.x;" : "=r"(n_clusters));
+#endif
     }
 
     unsigned char* acc = smem;                                  // accumulator region

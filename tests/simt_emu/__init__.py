@@ -1,0 +1,83 @@
+"""TEST INFRASTRUCTURE: runs the CUDA kernel's source (paper_2607_04067_b200/csrc/hough_kernel.cuh) on the CPU under a
+small SIMT emulator (simt_shim.h: fibers, barriers, warp collectives, guarded shared memory), so that the `-m "not
+gpu"` tests can compare the kernel's LOGIC with the oracle without a GPU.  Not a product path and not a parity claim:
+the product library never loads this, and only the GPU tests say anything about the device code itself.
+
+The launch shape and the shared-memory layout are asked from the product's own planner (hough_plan_describe), the
+tame bounds from hough_debug_tame_bounds, so the emulated launch is the one hough_run would make."""
+import os
+import struct
+import subprocess
+import tempfile
+
+import numpy as np
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+ROOT = os.path.dirname(os.path.dirname(HERE))
+SOURCES = [os.path.join(HERE, "emu_main.cpp"), os.path.join(HERE, "simt_shim.h"),
+           os.path.join(ROOT, "paper_2607_04067_b200", "csrc", "hough_kernel.cuh"), os.path.join(ROOT, "include", "hough.h"),
+           os.path.abspath(__file__)]
+FLAGS = ["-O1", "-g", "-std=c++17", "-ffp-contract=off", "-fno-fast-math", "-DHOUGH_HOST_EMU", "-Wno-unused-variable"]
+
+
+def exe_path(debug_bounds: bool) -> str:
+    return os.path.join(HERE, "hough_emu_dbg" if debug_bounds else "hough_emu")
+
+
+def build(debug_bounds: bool = False, force: bool = False) -> str:
+    exe = exe_path(debug_bounds)
+    if not force and os.path.exists(exe) and all(os.path.getmtime(s) <= os.path.getmtime(exe) for s in SOURCES):
+        return exe
+    tmp = exe + ".tmp.%d" % os.getpid()
+    subprocess.check_call(["g++", *FLAGS, *(["-DHOUGH_DEBUG_BOUNDS"] if debug_bounds else []), "-o", tmp, SOURCES[0]])
+    os.replace(tmp, exe)
+    return exe
+
+
+def run(xy, off, n_theta, n_rho, rho_max, threshold, window, table, max_peaks=64, acc_dtype="u16", accum=True,
+        conformal_scale=1, cluster_size=0, ctas_per_sm=0, vote_path=0, grid_clusters=0, debug_bounds=False, timeout=600):
+    """Same arguments and result keys as tests/test_parity_gpu.py::gpu_run."""
+    import paper_2607_04067_b200 as hb
+    xy = np.ascontiguousarray(xy, dtype=np.float32).reshape(-1, 2)
+    off = np.ascontiguousarray(off, dtype=np.int32)
+    n_events, n_total = len(off) - 1, len(xy)
+    acc = {"auto": hb.HOUGH_ACC_AUTO, "u16": hb.HOUGH_ACC_U16, "u32": hb.HOUGH_ACC_U32}[acc_dtype]
+    plan = hb.hough_plan_describe(n_theta, n_rho, acc, cluster_size=cluster_size, ctas_per_sm=ctas_per_sm)
+    fields = [plan[k] for k in hb.PLAN_FIELDS]
+    c, s = (np.ascontiguousarray(t, dtype=np.float32) for t in table)
+    tab = np.concatenate([np.abs(c), np.abs(s)])
+    nz = tab[tab > 0]
+    rho_max32 = float(np.float32(rho_max))
+    tame, ftz_min = hb.hough_debug_tame_bounds(n_rho, rho_max32, float(tab.max()), float(nz.min()) if nz.size else 0.0)
+    inv = np.float32(float(n_rho) / (2.0 * rho_max32))
+    head = [n_theta, n_rho, threshold, window, max_peaks, int(plan["acc_bits"] == 16), int(plan["cluster_size"] > 1),
+            plan["cols_per_lane"], plan["cluster_size"], plan["threads"], plan["smem_bytes"], int(vote_path == 1),
+            n_events, n_total, 1, int(accum), grid_clusters, 0, 0, 0]
+    with tempfile.TemporaryDirectory() as d:
+        fin, fout = os.path.join(d, "in.bin"), os.path.join(d, "out.bin")
+        with open(fin, "wb") as f:
+            f.write(struct.pack("<20i", *head))
+            f.write(struct.pack("<26i", *fields))
+            f.write(struct.pack("<5f", rho_max32, float(inv), float(conformal_scale), tame, ftz_min))
+            f.write(c.tobytes()); f.write(s.tobytes()); f.write(off.tobytes()); f.write(xy.tobytes())
+        r = subprocess.run([build(debug_bounds), fin, fout], capture_output=True, text=True, timeout=timeout)
+        if r.returncode != 0:
+            raise RuntimeError("hough_emu failed (rc %d): %s" % (r.returncode, r.stderr.strip()[-400:]))
+        raw = open(fout, "rb").read()
+    o = 0
+    def take(n, dtype):
+        nonlocal o
+        a = np.frombuffer(raw, dtype=dtype, count=n, offset=o)
+        o += a.nbytes
+        return a
+    res = {"keep": take(n_total, np.uint8),
+           "peaks": take(n_events * max_peaks * 2, np.int32).reshape(n_events, max_peaks, 2),
+           "counts": take(2 * n_events, np.int32).reshape(n_events, 2),
+           "kept_xy": take(2 * n_total, np.float32).reshape(n_total, 2),
+           "kept_idx": take(n_total, np.int32)}
+    if accum:
+        res["accum"] = take(n_events * n_theta * n_rho, np.int32).reshape(n_events, n_theta, n_rho)
+    res["peaks3"] = hb.unpack_peaks(res["peaks"])
+    res["info"] = {"CLUSTER_SIZE": plan["cluster_size"], "THREADS": plan["threads"], "SMEM_BYTES": plan["smem_bytes"],
+                   "ACC_BITS": plan["acc_bits"], "CHUNK_HITS": plan["chunk_hits"]}
+    return res

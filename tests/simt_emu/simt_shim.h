@@ -1,0 +1,290 @@
+// simt_shim.h -- TEST INFRASTRUCTURE.  A small single-OS-thread SIMT emulator that lets g++ compile
+// paper_2607_04067_b200/csrc/hough_kernel.cuh (with -DHOUGH_HOST_EMU) and execute it on the CPU: every CUDA
+// thread of a cluster is a fiber (ucontext); __syncthreads, cluster.sync and the full-mask warp collectives are
+// barriers at which a fiber yields; shared memory is one guarded buffer per CTA; shared atomics are plain
+// read-modify-writes (fibers never run concurrently).  It checks the kernel's LOGIC (indexing, phase order,
+// bounds) against the oracle without a GPU; it says nothing about races, PTX semantics or speed.
+#pragma once
+#include <sys/mman.h>
+#include <ucontext.h>
+#include <unistd.h>
+
+#include <cmath>
+#include <cstdint>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <vector>
+
+#define __global__
+#define __device__
+#define __host__
+#define __forceinline__ inline
+#define __launch_bounds__(...)
+#define __grid_constant__
+#define __align__(n) alignas(n)
+
+struct float2 { float x, y; };
+struct float4 { float x, y, z, w; };
+struct alignas(16) uint4 { unsigned x, y, z, w; };
+struct dim3 { unsigned x = 1, y = 1, z = 1; };
+inline float2 make_float2(float x, float y) { return float2{x, y}; }
+inline uint4 make_uint4(unsigned x, unsigned y, unsigned z, unsigned w) { return uint4{x, y, z, w}; }
+
+namespace emu {
+
+[[noreturn]] inline void die(const char* msg) {
+    fprintf(stderr, "simt_emu: %s\n", msg);
+    fflush(stderr);
+    _exit(3);
+}
+
+// A buffer whose END sits on a page boundary followed by an inaccessible page, and whose start is preceded by one:
+// an access past the end faults at once, one before the start faults within a page.
+struct Guarded {
+    unsigned char* base = nullptr;   // mmap base
+    size_t map_bytes = 0;
+    unsigned char* ptr = nullptr;    // user pointer
+    size_t bytes = 0;
+    void alloc(size_t n) {
+        const size_t pg = (size_t)sysconf(_SC_PAGESIZE);
+        bytes = n;
+        const size_t body = (n + pg - 1) / pg * pg;
+        map_bytes = body + 2 * pg;
+        base = (unsigned char*)mmap(nullptr, map_bytes, PROT_READ | PROT_WRITE, MAP_PRIVATE | MAP_ANONYMOUS, -1, 0);
+        if (base == MAP_FAILED) die("mmap failed");
+        mprotect(base, pg, PROT_NONE);
+        mprotect(base + pg + body, pg, PROT_NONE);
+        ptr = base + pg + body - n;               // n is a multiple of 16 for shared memory, so ptr is 16-byte aligned there
+    }
+    void release() { if (base) munmap(base, map_bytes); base = nullptr; }
+};
+
+struct Barrier {
+    int expected = 0, arrived = 0;
+    unsigned gen = 0;
+    int acc_and = 1, acc_or = 0, acc_cnt = 0;
+    int res_and = 1, res_or = 0, res_cnt = 0;
+};
+
+struct Warp {
+    int arrived = 0;
+    unsigned gen = 0;
+    unsigned vals[2][32];
+};
+
+struct Cta {
+    Guarded smem;
+    int rank = 0;
+    dim3 bidx;
+    Barrier bar;
+    std::vector<Warp> warps;
+};
+
+struct Fiber {
+    ucontext_t ctx;
+    std::vector<unsigned char> stack;
+    dim3 tidx;
+    Cta* cta = nullptr;
+    bool done = false;
+    unsigned long progress = 0;      // bumped whenever the fiber gets past a wait
+};
+
+struct Grid {
+    dim3 bdim, gdim;
+    int csize = 1, cluster = 0, n_clusters_ = 1;
+    std::vector<Cta> ctas;           // the CTAs of the cluster being run
+    Barrier cluster_bar;
+    ucontext_t sched;
+    void (*entry)() = nullptr;
+};
+
+inline Grid g;
+inline Fiber* cur = nullptr;
+
+inline void yield() {
+    Fiber* me = cur;
+    swapcontext(&me->ctx, &g.sched);
+}
+
+inline void wait_barrier(Barrier& b, int pred, int& r_and, int& r_or, int& r_cnt) {
+    const unsigned gen = b.gen;
+    b.acc_and &= pred ? 1 : 0;
+    b.acc_or |= pred ? 1 : 0;
+    b.acc_cnt += pred ? 1 : 0;
+    if (++b.arrived == b.expected) {
+        b.res_and = b.acc_and; b.res_or = b.acc_or; b.res_cnt = b.acc_cnt;
+        b.acc_and = 1; b.acc_or = 0; b.acc_cnt = 0;
+        b.arrived = 0;
+        ++b.gen;
+    } else {
+        while (b.gen == gen) yield();
+    }
+    ++cur->progress;
+    r_and = b.res_and; r_or = b.res_or; r_cnt = b.res_cnt;
+}
+
+// full-mask warp collective: every lane deposits `v`, all wait, every lane may read any lane's value
+inline const unsigned* warp_exchange(unsigned v) {
+    Cta* c = cur->cta;
+    Warp& w = c->warps[cur->tidx.x >> 5];
+    const unsigned gen = w.gen;
+    unsigned* buf = w.vals[gen & 1];
+    buf[cur->tidx.x & 31] = v;
+    if (++w.arrived == 32) {
+        w.arrived = 0;
+        ++w.gen;
+    } else {
+        while (w.gen == gen) yield();
+    }
+    ++cur->progress;
+    return buf;
+}
+
+constexpr unsigned SHARED_WINDOW = 0x01000000u;   // what __cvta_generic_to_shared returns for the first byte
+inline unsigned char* shared_ptr(unsigned saddr) {
+    const unsigned off = saddr - SHARED_WINDOW;
+    if ((size_t)off + 4 > cur->cta->smem.bytes) die("shared-window address outside the CTA's shared memory");
+    return cur->cta->smem.ptr + off;
+}
+inline unsigned char* dyn_smem() { return cur->cta->smem.ptr; }
+inline int cluster_id() { return g.cluster; }
+inline int n_clusters() { return g.n_clusters_; }
+
+inline float ftz(float x) { return std::fpclassify(x) == FP_SUBNORMAL ? std::copysign(0.0f, x) : x; }
+
+inline void fiber_main() {
+    g.entry();
+    cur->done = true;
+    swapcontext(&cur->ctx, &g.sched);
+}
+
+// Runs one cluster (csize CTAs of `threads` threads, `smem_bytes` each) to completion.
+inline void run_cluster(int cluster, int n_clusters, int csize, int threads, size_t smem_bytes, void (*entry)()) {
+    g.bdim.x = (unsigned)threads;
+    g.gdim.x = (unsigned)(n_clusters * csize);
+    g.csize = csize; g.cluster = cluster; g.n_clusters_ = n_clusters; g.entry = entry;
+    g.ctas.assign((size_t)csize, Cta());
+    g.cluster_bar = Barrier();
+    g.cluster_bar.expected = csize * threads;
+    std::vector<Fiber> fibers((size_t)csize * threads);
+    for (int r = 0; r < csize; ++r) {
+        Cta& c = g.ctas[r];
+        c.smem.alloc(smem_bytes);
+        memset(c.smem.ptr, 0xCD, smem_bytes);       // shared memory starts as garbage, as on the device
+        c.rank = r;
+        c.bidx.x = (unsigned)(cluster * csize + r);
+        c.bar.expected = threads;
+        c.warps.assign((size_t)threads / 32, Warp());
+        for (int t = 0; t < threads; ++t) {
+            Fiber& f = fibers[(size_t)r * threads + t];
+            f.stack.resize(48 * 1024);
+            f.tidx.x = (unsigned)t;
+            f.cta = &c;
+            getcontext(&f.ctx);
+            f.ctx.uc_stack.ss_sp = f.stack.data();
+            f.ctx.uc_stack.ss_size = f.stack.size();
+            f.ctx.uc_link = nullptr;
+            makecontext(&f.ctx, (void (*)())fiber_main, 0);
+        }
+    }
+    size_t live = fibers.size();
+    while (live) {
+        unsigned long before = 0, after = 0;
+        for (auto& f : fibers) before += f.progress;
+        size_t finished_now = 0;
+        for (auto& f : fibers) {
+            if (f.done) continue;
+            cur = &f;
+            swapcontext(&g.sched, &f.ctx);
+            if (f.done) { ++finished_now; --live; }
+        }
+        for (auto& f : fibers) after += f.progress;
+        if (after == before && finished_now == 0) die("deadlock: a barrier or warp collective was not reached by every thread");
+    }
+    cur = nullptr;
+    for (auto& c : g.ctas) c.smem.release();
+}
+
+}  // namespace emu
+
+// ---------------------------------------------------------------- the CUDA names the kernel uses
+#define threadIdx (emu::cur->tidx)
+#define blockIdx (emu::cur->cta->bidx)
+#define blockDim (emu::g.bdim)
+#define gridDim (emu::g.gdim)
+#define HOUGH_DYN_SMEM(name) unsigned char* name = emu::dyn_smem()
+
+inline void __syncthreads() { int a, o, c; emu::wait_barrier(emu::cur->cta->bar, 1, a, o, c); }
+inline int __syncthreads_and(int p) { int a, o, c; emu::wait_barrier(emu::cur->cta->bar, p, a, o, c); return a; }
+inline int __syncthreads_or(int p) { int a, o, c; emu::wait_barrier(emu::cur->cta->bar, p, a, o, c); return o; }
+inline int __syncthreads_count(int p) { int a, o, c; emu::wait_barrier(emu::cur->cta->bar, p, a, o, c); return c; }
+inline void __threadfence() {}
+
+inline void need_full_mask(unsigned m) { if (m != 0xffffffffu) emu::die("only full-mask warp collectives are emulated"); }
+inline int __shfl_sync(unsigned m, int v, int src) { need_full_mask(m); return (int)emu::warp_exchange((unsigned)v)[src & 31]; }
+inline int __shfl_up_sync(unsigned m, int v, int d) {
+    need_full_mask(m);
+    const int lane = (int)(emu::cur->tidx.x & 31);
+    const unsigned* b = emu::warp_exchange((unsigned)v);
+    return lane >= d ? (int)b[lane - d] : v;
+}
+inline unsigned __ballot_sync(unsigned m, int p) {
+    need_full_mask(m);
+    const unsigned* b = emu::warp_exchange(p ? 1u : 0u);
+    unsigned r = 0;
+    for (int l = 0; l < 32; ++l) r |= (b[l] & 1u) << l;
+    return r;
+}
+inline int __all_sync(unsigned m, int p) { return __ballot_sync(m, p) == 0xffffffffu; }
+
+inline unsigned atomicAdd(unsigned* p, unsigned v) { unsigned o = *p; *p = o + v; return o; }
+inline int atomicAdd(int* p, int v) { int o = *p; *p = o + v; return o; }
+template <class T> inline T __ldg(const T* p) { return *p; }
+inline size_t __cvta_generic_to_shared(const void* p) {
+    const ptrdiff_t off = (const unsigned char*)p - emu::cur->cta->smem.ptr;
+    if (off < 0 || (size_t)off >= emu::cur->cta->smem.bytes) emu::die("cvta of a pointer outside the CTA's shared memory");
+    return (size_t)emu::SHARED_WINDOW + (size_t)off;
+}
+
+inline unsigned __float_as_uint(float f) { unsigned u; memcpy(&u, &f, 4); return u; }
+inline float __uint_as_float(unsigned u) { float f; memcpy(&f, &u, 4); return f; }
+// one rounding per operation: this file is compiled with -ffp-contract=off and without fast-math
+inline float __fmul_rn(float a, float b) { volatile float r = a * b; return r; }
+inline float __fadd_rn(float a, float b) { volatile float r = a + b; return r; }
+inline float __fdiv_rn(float a, float b) { volatile float r = a / b; return r; }
+inline float __fadd_rd(float a, float b) {        // round toward minus infinity: exact in double, then step down if needed
+    const double s = (double)a + (double)b;
+    float r = (float)s;
+    if (std::isfinite(r) && (double)r > s) r = std::nextafterf(r, -INFINITY);
+    return r;
+}
+inline int __popc(unsigned x) { return __builtin_popcount(x); }
+inline int __ffs(unsigned x) { return __builtin_ffs((int)x); }
+inline unsigned umax3(unsigned a, unsigned b, unsigned c) { return a > b ? (a > c ? a : c) : (b > c ? b : c); }
+inline unsigned __vimax3_u32(unsigned a, unsigned b, unsigned c) { return umax3(a, b, c); }
+inline unsigned __vimax3_u16x2(unsigned a, unsigned b, unsigned c) {
+    return umax3(a & 0xFFFFu, b & 0xFFFFu, c & 0xFFFFu) | (umax3(a >> 16, b >> 16, c >> 16) << 16);
+}
+inline unsigned __vibmax_u16x2(unsigned a, unsigned b, bool* hi, bool* lo) {   // per-half max; *hi / *lo: a's half is >= b's
+    *lo = (a & 0xFFFFu) >= (b & 0xFFFFu);
+    *hi = (a >> 16) >= (b >> 16);
+    return ((*lo ? a : b) & 0xFFFFu) | ((*hi ? a : b) & 0xFFFF0000u);
+}
+template <class T> inline T min(T a, T b) { return a < b ? a : b; }
+template <class T> inline T max(T a, T b) { return a > b ? a : b; }
+inline unsigned min(unsigned a, int b) { return a < (unsigned)b ? a : (unsigned)b; }
+
+namespace cooperative_groups {
+struct cluster_group {
+    unsigned block_rank() const { return (unsigned)emu::cur->cta->rank; }
+    void sync() const { int a, o, c; emu::wait_barrier(emu::g.cluster_bar, 1, a, o, c); }
+    void* map_shared_rank(void* p, int rank) const {
+        const ptrdiff_t off = (unsigned char*)p - emu::cur->cta->smem.ptr;
+        if (off < 0 || (size_t)off >= emu::cur->cta->smem.bytes) emu::die("map_shared_rank of a pointer outside shared memory");
+        if (rank < 0 || rank >= emu::g.csize) emu::die("map_shared_rank: bad rank");
+        return emu::g.ctas[(size_t)rank].smem.ptr + off;
+    }
+};
+inline cluster_group this_cluster() { return cluster_group(); }
+}  // namespace cooperative_groups

@@ -12,11 +12,17 @@ prints ONE JSON line (contract in DESIGN.md "Measurement").
                         step is timed by its own CUDA-event pair on the launching
                         stream and L2 is flushed (256 MiB write) before each step
   e2e                 : the same metric through hough_run_host() with pinned HOST
-                        buffers: H2D of hits+offsets and D2H of mask, peaks,
-                        counts and the compacted hits inside the timed region
+                        buffers: H2D of hits+offsets and D2H of the results inside
+                        the timed region
+                        (lean: mask + peaks + counts come back; e2e.full adds the
+                        compacted hits)
   roofline            : achieved in-range votes/s of the one kernel against the
                         shared-atomic rate measured live on this GPU, plus the
                         HBM term (north_star: the slower of the two binds)
+  all_configs         : events/s, Gvotes/s and roofline fraction of EVERY BASELINE.json
+                        configuration (0-3, the 100k-event sweep at 180x256 and at the
+                        360x512 cluster grid), >= 20 CUDA-event-timed steps each
+  multi_stream        : the sweep in batches of 1k/10k/100k events on 1/2/4 streams
   cpu_baseline        : the oracle, as it stands, on the host cores (rank 0, N=1)
 
 --impl reference times the oracle (the only reference this tier has) and is
@@ -51,7 +57,11 @@ def parse_args():
     ap.add_argument("--no-flush", action="store_true", help="do not flush L2 between steps (diagnostic only)")
     ap.add_argument("--ctas-per-sm", type=int, default=0)
     ap.add_argument("--cluster", type=int, default=0)
-    ap.add_argument("--vote-path", type=int, default=0, help="HOUGH_OPT_VOTE_PATH (0 packed fast, 1 exact slow)")
+    ap.add_argument("--vote-path", type=int, default=0,
+                    help="HOUGH_OPT_VOTE_PATH (0 packed fast, 1 exact slow; 2/3 = phase-skipping diagnostics of the bench-only diag build)")
+    ap.add_argument("--no-all-configs", action="store_true", help="skip the all_configs / multi_stream blocks (headline only)")
+    ap.add_argument("--config-steps", type=int, default=20, help="timed steps per configuration in the all_configs block")
+    ap.add_argument("--sweep-events", type=int, default=100000, help="events of the config-4 sweep (all_configs, multi_stream)")
     return ap.parse_args()
 
 
@@ -193,23 +203,151 @@ def hbm_peak():
         return 6650.0, "fallback (B200_PROFILING.md)"
 
 
-def dram_traffic(workload_name):
-    """dram__bytes_read.sum + dram__bytes_write.sum per launch of the kernel, from the committed ncu capture
-    (profiles/dram_traffic.csv); None when this workload has no capture."""
-    try:
-        import csv
-        with open(os.path.join(ROOT, "profiles", "dram_traffic.csv")) as f:
-            for row in csv.DictReader(f):
-                if row["workload"] == workload_name:
-                    return int(row["dram_bytes_read_per_launch"]) + int(row["dram_bytes_write_per_launch"])
-    except Exception:  # noqa: BLE001
-        pass
-    return None
+class Workbench:
+    """One workload resident on the device: inputs, outputs, handle.  Marshalling and timing only."""
+
+    def __init__(self, hb, si, torch, dev, cfg, n_events, first_event=0, cluster=0, ctas_per_sm=0, vote_path=0):
+        self.hb, self.torch, self.dev = hb, torch, dev
+        self.w = w = si.config(cfg)
+        self.n_events = n_events
+        self.xy, self.off, _ = si.generate(w, n_events, first_event=first_event)
+        self.n_total = len(self.xy)
+        self.table = si.trig_table(w.n_theta)
+        self.h = hb.Hough(w.n_theta, w.n_rho, w.rho_max, w.threshold, w.window, max_peaks=w.max_peaks, acc_dtype=w.acc_dtype,
+                          cluster_size=cluster, ctas_per_sm=ctas_per_sm, trig_table=self.table)
+        if vote_path:
+            hb.hough_set_option(self.h.ctx, hb.HOUGH_OPT_VOTE_PATH, vote_path)
+        self.info = {k: self.h.info(getattr(hb, "HOUGH_INFO_" + k)) for k in
+                     ("CLUSTER_SIZE", "THREADS", "SMEM_BYTES", "CTAS_PER_SM", "GRID_MAX", "ACC_BITS", "CHUNK_HITS", "SM_COUNT")}
+        self.d_xy = torch.from_numpy(self.xy).to(dev)
+        self.d_off = torch.from_numpy(self.off).to(dev)
+        self.out = self.h.alloc_outputs(self.n_total, n_events, dev, kept=True, accum=False)
+        self.pairs = self.n_total * w.n_theta
+
+    def step(self, stream):
+        o = self.out
+        self.hb.hough_run_ex(self.h.ctx, self.d_xy, self.d_off, self.n_events, o["keep"], o["peaks"], o["counts"],
+                             o["kept_xy"], o["kept_idx"], None, stream)
+
+    def timed(self, steps, warmup, flush, stream):
+        """`steps` launches, each with its own CUDA-event pair on the launching stream (ms per step)."""
+        torch = self.torch
+        for _ in range(max(warmup, 3)):
+            if flush is not None:
+                flush.zero_()
+            self.step(stream)
+        torch.cuda.synchronize()
+        evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+        for a, b in evs:
+            if flush is not None:
+                flush.zero_()
+            a.record(stream)
+            self.step(stream)
+            b.record(stream)
+        torch.cuda.synchronize()
+        import numpy as np
+        return np.array([a.elapsed_time(b) for a, b in evs], dtype=np.float64)
+
+    def in_range_votes(self, sample_events=None):
+        """V_in = sum of all accumulator cells (one shared atomic per in-range vote: the roofline's unit), from the
+        kernel's own dump, untimed.  With sample_events the fraction of a leading sample is scaled to the batch."""
+        torch = self.torch
+        n_ev = self.n_events if sample_events is None else min(sample_events, self.n_events)
+        v_in, step_ev = 0, 125
+        for e0 in range(0, n_ev, step_ev):
+            e1 = min(n_ev, e0 + step_ev)
+            sub_off = (self.d_off[e0:e1 + 1] - self.d_off[e0]).contiguous()
+            sub_xy = self.d_xy[int(self.off[e0]):int(self.off[e1])]
+            o = self.h.run(sub_xy, sub_off, kept=False, accum=True)
+            v_in += int(o["accum"].sum(dtype=torch.int64).item())
+            del o
+        if n_ev == self.n_events:
+            return v_in, "exact"
+        frac = v_in / max(1, int(self.off[n_ev]) * self.w.n_theta)
+        return int(round(frac * self.pairs)), "in-range fraction of the first %d events x all pairs" % n_ev
+
+    def counts(self):
+        c = self.out["counts"].cpu()
+        return int(c[:, 1].sum().item()), int(c[:, 0].clamp(max=self.w.max_peaks).sum().item())
+
+    def alg_bytes(self):
+        n_kept, n_peaks = self.counts()
+        return 8 * self.n_total + 4 * (self.n_events + 1) + self.n_total + 12 * n_kept + 8 * n_peaks + 8 * self.n_events
+
+    def close(self):
+        self.h.close()
+
+
+def roofline_block(wb, t_kernel_s, v_in, v_in_how, atom_rate, hbm_gbs, hbm_src):
+    alg_bytes = wb.alg_bytes()
+    t_vote, t_hbm = v_in / atom_rate, alg_bytes / (hbm_gbs * 1e9)
+    return {
+        "bound": "alu", "pipe": "shared-memory atomics (ATOMS), one per in-range vote; the slower of the vote and HBM terms binds (north_star)",
+        "achieved": v_in / t_kernel_s / 1e9, "peak": atom_rate / 1e9, "unit": "Gvotes/s (in-range)",
+        "frac": max(t_vote, t_hbm) / t_kernel_s,
+        "traffic": None, "traffic_note": "no ncu capture of this commit in this run; see profiles/ for the last one and its commit",
+        "peak_source": "hough_bench_shared_atomics(variant 5) measured in this run: conflict-free 32-bit shared atomics, all SMs",
+        "algorithmic_votes_per_launch": v_in, "votes_counted": v_in_how, "algorithmic_bytes_per_launch": alg_bytes,
+        "t_vote_us": t_vote * 1e6, "t_hbm_us": t_hbm * 1e6, "t_kernel_us": t_kernel_s * 1e6,
+        "hbm": {"achieved": alg_bytes / t_kernel_s / 1e9, "peak": hbm_gbs, "unit": "GB/s", "frac": t_hbm / t_kernel_s, "peak_source": hbm_src},
+    }
+
+
+def config_line(wb, times_ms, v_in, v_in_how, atom_rate, hbm_gbs, hbm_src):
+    import numpy as np
+    ms = float(times_ms.mean())
+    t = ms * 1e-3
+    r = roofline_block(wb, t, v_in, v_in_how, atom_rate, hbm_gbs, hbm_src)
+    n_kept, _ = wb.counts()
+    return {"workload": wb.w.name, "events": wb.n_events, "hits": wb.n_total, "grid": "%dx%d %s" % (wb.w.n_theta, wb.w.n_rho, wb.w.acc_dtype),
+            "cluster_size": wb.info["CLUSTER_SIZE"], "threads": wb.info["THREADS"], "ctas_per_sm": wb.info["CTAS_PER_SM"],
+            "steps": int(len(times_ms)), "ms_per_step": ms, "ms_per_step_min": float(times_ms.min()), "ms_per_step_median": float(np.median(times_ms)),
+            "events_per_s": wb.n_events / t, "gvotes_per_s": wb.pairs / t / 1e9, "gvotes_in_range_per_s": v_in / t / 1e9,
+            "frac": r["frac"], "hbm_frac": r["hbm"]["frac"], "kept_fraction": n_kept / max(1, wb.n_total)}
+
+
+def multi_stream_sweep(wb, torch, batches=(1000, 10000, 100000), streams_list=(1, 2, 4), reps=3):
+    """BASELINE.json config 4: the sweep's events in batches of 1k / 10k / 100k on 1, 2 and 4 CUDA streams through ONE
+    handle (no per-run scratch; PAPER.md:90 batching, :204-210 batch scaling).  A sub-batch is a pointer offset into
+    the same device arrays (offsets are absolute), so nothing is copied.  Device time from a start event that every
+    stream waits on to the last stream's end event."""
+    hb, o = wb.hb, wb.out
+    res = []
+    pools = {n: [torch.cuda.Stream() for _ in range(n)] for n in streams_list}
+    main = torch.cuda.current_stream()
+    for B in batches:
+        if B > wb.n_events:
+            continue
+        for ns in streams_list:
+            st = pools[ns]
+            best = None
+            for rep in range(reps + 1):            # the first repetition is the warm-up
+                torch.cuda.synchronize()
+                start = torch.cuda.Event(enable_timing=True)
+                ends = [torch.cuda.Event(enable_timing=True) for _ in st]
+                start.record(main)
+                for s_ in st:
+                    s_.wait_event(start)
+                for bi, e0 in enumerate(range(0, wb.n_events, B)):
+                    e1 = min(wb.n_events, e0 + B)
+                    hb.hough_run_ex(wb.h.ctx, wb.d_xy, wb.d_off[e0:], e1 - e0, o["keep"], o["peaks"][e0:], o["counts"][e0:],
+                                    o["kept_xy"], o["kept_idx"], None, st[bi % ns])
+                for s_, ev in zip(st, ends):
+                    ev.record(s_)
+                torch.cuda.synchronize()
+                ms = max(start.elapsed_time(ev) for ev in ends)
+                if rep > 0:
+                    best = ms if best is None else min(best, ms)
+            res.append({"batch_events": B, "streams": ns, "launches": (wb.n_events + B - 1) // B, "ms_total": best,
+                        "events_per_s": wb.n_events / (best * 1e-3)})
+    return res
 
 
 def run_ours(args):
     import numpy as np
     import torch
+    if args.vote_path >= 2:
+        os.environ["HOUGH_B200_FLAVOR"] = "diag"     # the phase-skipping diagnostics live in a bench-only build
     import paper_2607_04067_b200 as hb
     import stcf_inputs as si
     from paper_2607_04067_b200 import shard
@@ -231,32 +369,18 @@ def run_ours(args):
     w = si.config(args.config)
     n_events = args.events or min(w.n_events, 1000)
     first_event, _ = shard.event_range(rank, world, n_events)             # every rank its own events
-    xy, off, _ = si.generate(w, n_events, first_event=first_event)
-    n_total = len(xy)
-    table = si.trig_table(w.n_theta)
-    h = hb.Hough(w.n_theta, w.n_rho, w.rho_max, w.threshold, w.window, max_peaks=w.max_peaks, acc_dtype=w.acc_dtype,
-                 cluster_size=args.cluster, ctas_per_sm=args.ctas_per_sm, trig_table=table)
-    if args.vote_path:
-        hb.hough_set_option(h.ctx, hb.HOUGH_OPT_VOTE_PATH, args.vote_path)
-    info = {k: h.info(getattr(hb, "HOUGH_INFO_" + k)) for k in
-            ("CLUSTER_SIZE", "THREADS", "SMEM_BYTES", "CTAS_PER_SM", "GRID_MAX", "ACC_BITS", "CHUNK_HITS", "SM_COUNT")}
+    wb = Workbench(hb, si, torch, dev, args.config, n_events, first_event, args.cluster, args.ctas_per_sm, args.vote_path)
+    xy, off, n_total, info, h = wb.xy, wb.off, wb.n_total, dict(wb.info), wb.h
     info["VOTE_PATH"] = args.vote_path
-    d_xy = torch.from_numpy(xy).to(dev)
-    d_off = torch.from_numpy(off).to(dev)
-    out = h.alloc_outputs(n_total, n_events, dev, kept=True, accum=False)
+    info["LIBRARY"] = os.path.basename(hb.lib_path())
     stream = torch.cuda.current_stream()
-
-    pairs = n_total * w.n_theta
     flush = None if args.no_flush else torch.empty(256 << 20, dtype=torch.uint8, device=dev)
 
-    def step():
-        hb.hough_run_ex(h.ctx, d_xy, d_off, n_events, out["keep"], out["peaks"], out["counts"],
-                        out["kept_xy"], out["kept_idx"], None, stream)
-
+    # ---- the headline: `steps` timed launches, cold L2, clocks sampled during the timed region
     for _ in range(max(args.warmup, 3)):
         if flush is not None:
             flush.zero_()
-        step()
+        wb.step(stream)
     torch.cuda.synchronize()
     launches0 = h.info(hb.HOUGH_INFO_LAUNCHES)
     evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
@@ -269,7 +393,7 @@ def run_ours(args):
         if flush is not None:
             flush.zero_()
         a.record(stream)
-        step()
+        wb.step(stream)
         b.record(stream)
     torch.cuda.synchronize()
     barrier()
@@ -283,12 +407,14 @@ def run_ours(args):
     a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     a.record(stream)
     for _ in range(args.steps):
-        step()
+        wb.step(stream)
     b.record(stream)
     torch.cuda.synchronize()
     warm_ms = a.elapsed_time(b) / args.steps
 
-    # ---- end to end through hough_run_host: pinned host buffers, copies inside the timed region
+    # ---- end to end through hough_run_host: pinned host buffers, copies inside the timed region.
+    # "lean" (headline e2e): H2D hits + offsets, D2H mask + peaks + counts -- what a host consumer that still holds its
+    # hits needs; "full" adds the compacted hits and their indices (full-length arrays, reading Q11).
     h_xy, h_off = torch.from_numpy(xy).pin_memory(), torch.from_numpy(off).pin_memory()
     h_keep = torch.empty(n_total, dtype=torch.uint8).pin_memory()
     h_peaks = torch.zeros((n_events, w.max_peaks, 2), dtype=torch.int32).pin_memory()
@@ -296,63 +422,42 @@ def run_ours(args):
     h_kxy = torch.empty((n_total, 2), dtype=torch.float32).pin_memory()
     h_kidx = torch.empty(n_total, dtype=torch.int32).pin_memory()
     e2e_steps = min(args.steps, 50)
-    for _ in range(3):
-        hb.hough_run_host(h.ctx, h_xy, h_off, n_events, h_keep, h_peaks, h_counts, h_kxy, h_kidx, stream)
-    torch.cuda.synchronize()
-    barrier()
-    e2e_ms = 0.0
-    for _ in range(e2e_steps):
-        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        a.record(stream)
-        hb.hough_run_host(h.ctx, h_xy, h_off, n_events, h_keep, h_peaks, h_counts, h_kxy, h_kidx, stream)
-        b.record(stream)
-        b.synchronize()               # the caller reads the results on the host here
-        e2e_ms += a.elapsed_time(b)
-    barrier()
-    n_kept = int(h_counts[:, 1].sum().item())
-    n_peaks = int(h_counts[:, 0].clamp(max=w.max_peaks).sum().item())
+    e2e = {}
+    for mode, kx, ki in (("lean", None, None), ("full", h_kxy, h_kidx)):
+        for _ in range(3):
+            hb.hough_run_host(h.ctx, h_xy, h_off, n_events, h_keep, h_peaks, h_counts, kx, ki, stream)
+        torch.cuda.synchronize()
+        barrier()
+        ms_sum = 0.0
+        for _ in range(e2e_steps):
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(stream)
+            hb.hough_run_host(h.ctx, h_xy, h_off, n_events, h_keep, h_peaks, h_counts, kx, ki, stream)
+            b.record(stream)
+            b.synchronize()               # the caller reads the results on the host here
+            ms_sum += a.elapsed_time(b)
+        barrier()
+        d2h = h_keep.numel() + h_peaks.numel() * 4 + h_counts.numel() * 4 + (0 if kx is None else h_kxy.numel() * 4 + h_kidx.numel() * 4)
+        e2e[mode] = (ms_sum, d2h)
     h2d = h_xy.numel() * 4 + h_off.numel() * 4
-    d2h = h_keep.numel() + h_peaks.numel() * 4 + h_counts.numel() * 4 + h_kxy.numel() * 4 + h_kidx.numel() * 4
 
-    # in-range votes V_in = sum of all accumulator cells (the roofline's unit), from the kernel's own dump;
-    # untimed, and after the timed regions so that a profiler's first hough launches are the real ones
-    v_in = 0
-    step_ev = 125
-    for e0 in range(0, n_events, step_ev):
-        e1 = min(n_events, e0 + step_ev)
-        sub_off = (d_off[e0:e1 + 1] - d_off[e0]).contiguous()
-        sub_xy = d_xy[int(off[e0]):int(off[e1])]
-        o = h.run(sub_xy, sub_off, kept=False, accum=True)
-        v_in += int(o["accum"].sum(dtype=torch.int64).item())
-        del o
-
+    v_in, v_in_how = wb.in_range_votes(None if n_events <= 5000 else 2000)
 
     # ---- max over ranks (plumbing only)
-    total_ms, e2e_ms, warm_ms = shard.max_over_ranks([total_ms, e2e_ms, warm_ms], device=dev)
+    total_ms, e2e_lean_ms, e2e_full_ms, warm_ms = shard.max_over_ranks([total_ms, e2e["lean"][0], e2e["full"][0], warm_ms], device=dev)
     ms_per_step = total_ms / args.steps
     value = shard.job_throughput(n_events, world, ms_per_step)
-    e2e_value = shard.job_throughput(n_events, world, e2e_ms / e2e_steps)
 
     # ---- roofline of the one kernel (per launch, this rank)
     atom_rate = hb.hough_bench_shared_atomics(5, 1, 1024, 20000)          # conflict-free ATOMS/s, all SMs, measured now
     hbm_gbs, hbm_src = hbm_peak()
-    alg_bytes = 8 * n_total + 4 * (n_events + 1) + n_total + 12 * n_kept + 8 * n_peaks + 8 * n_events
     t_kernel = ms_per_step * 1e-3
-    t_vote, t_hbm = v_in / atom_rate, alg_bytes / (hbm_gbs * 1e9)
-    roof = {
-        "bound": "alu", "pipe": "shared-memory atomics (ATOMS), one per in-range vote; the slower of the vote and HBM terms binds (north_star)",
-        "achieved": v_in / t_kernel / 1e9, "peak": atom_rate / 1e9, "unit": "Gvotes/s (in-range)",
-        "frac": max(t_vote, t_hbm) / t_kernel, "traffic": dram_traffic(w.name),
-        "peak_source": "hough_bench_shared_atomics(variant 5) measured in this run: conflict-free 32-bit shared atomics, all SMs",
-        "algorithmic_votes_per_launch": v_in, "algorithmic_bytes_per_launch": alg_bytes,
-        "t_vote_us": t_vote * 1e6, "t_hbm_us": t_hbm * 1e6, "t_kernel_us": t_kernel * 1e6,
-        # diagnostic third ceiling: 10.3 issue slots per (hit, theta) vote, 4 slots per clock per SM
-        "issue_slot_ceiling": {"slots_per_vote": 10.3, "peak": info["SM_COUNT"] * (clocks.get("sm_mhz") or 1965) * 1e6 * 128 / 10.3 / 1e9,
-                               "achieved": pairs / t_kernel / 1e9, "unit": "Gvotes/s (hit x theta)",
-                               "frac": (pairs / t_kernel) / (info["SM_COUNT"] * (clocks.get("sm_mhz") or 1965) * 1e6 * 128 / 10.3),
-                               "source": "profiles/r01_microbench_voteloop.md"},
-        "hbm": {"achieved": alg_bytes / t_kernel / 1e9, "peak": hbm_gbs, "unit": "GB/s", "frac": t_hbm / t_kernel, "peak_source": hbm_src},
-    }
+    roof = roofline_block(wb, t_kernel, v_in, v_in_how, atom_rate, hbm_gbs, hbm_src)
+    # diagnostic third ceiling: the voting loop's own instruction sequence, alone on the SMs, measured now
+    probe = hb.hough_bench_vote_loop(15, 6, 2, 512, 20)
+    roof["vote_loop_probe"] = {"lane_votes_per_s_incl_padding": probe, "unit": "hit x theta pairs/s, 192 padded columns per 180",
+                               "kernel_vs_probe": (wb.pairs * 192.0 / 180.0 / t_kernel) / probe if w.n_theta == 180 else None,
+                               "probe_vs_atomic_peak": probe / atom_rate}
 
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
@@ -362,25 +467,49 @@ def run_ours(args):
             "l2": "cold: 256 MiB write between steps" if flush is not None else "warm",
             "hits_per_gpu": n_total, "launch": info, "ms_per_step_warm_l2_back_to_back": warm_ms,
             "ms_per_step_min": float(times.min()), "ms_per_step_median": float(np.median(times)),
-            "kept_fraction": n_kept / max(1, n_total), "wall_s_timed_region": t_wall}),
-        "gvotes_per_s": world * pairs / t_kernel / 1e9,
+            "kept_fraction": wb.counts()[0] / max(1, n_total), "wall_s_timed_region": t_wall}),
+        "gvotes_per_s": world * wb.pairs / t_kernel / 1e9,
         "gvotes_in_range_per_s": world * v_in / t_kernel / 1e9,
         "roofline": roof, "clocks": clocks,
-        "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
-                "ms_per_step": e2e_ms / e2e_steps, "steps": e2e_steps},
+        "e2e": {"value": shard.job_throughput(n_events, world, e2e_lean_ms / e2e_steps), "unit": UNIT,
+                "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": e2e["lean"][1], "ms_per_step": e2e_lean_ms / e2e_steps, "steps": e2e_steps,
+                "returns": "keep mask + peaks + counts (lean mode of hough_run_host)",
+                "full": {"value": shard.job_throughput(n_events, world, e2e_full_ms / e2e_steps), "d2h_bytes_per_step": e2e["full"][1],
+                         "ms_per_step": e2e_full_ms / e2e_steps, "returns": "lean + kept_xy + kept_idx (full-length arrays)"}},
         "gpu_launches": int(launches),
     }
+    wb.close()
+
+    # ---- every configuration of BASELINE.json in the same line (rank 0, single GPU; north_star: "events/s reported for every config")
+    if rank == 0 and world == 1 and not args.no_all_configs and not args.vote_path:
+        allc = []
+        for cfg, nev, cl in ((0, 16, 0), (1, 1000, 0), (2, 1000, 0), (3, 1000, 0), (4, args.sweep_events, 0), (5, args.sweep_events, 0)):
+            b2 = Workbench(hb, si, torch, dev, cfg, nev)
+            fl = flush if b2.n_total * 8 < (96 << 20) else None       # inputs larger than L2 need no flush
+            steps2 = args.config_steps if nev <= 1000 else max(5, args.config_steps // 4)
+            t2 = b2.timed(steps2, 3, fl, stream)
+            v2, how2 = b2.in_range_votes(None if nev <= 1000 else 2000)
+            c = config_line(b2, t2, v2, how2, atom_rate, hbm_gbs, hbm_src)
+            c["l2"] = "cold: 256 MiB write between steps" if fl is not None else "inputs (%d MB) exceed L2" % (b2.n_total * 8 >> 20)
+            allc.append(c)
+            if cfg == 4:
+                line["multi_stream"] = {"workload": b2.w.name, "events": nev, "what": "whole sweep in batches on 1/2/4 streams through one handle",
+                                        "runs": multi_stream_sweep(b2, torch)}
+            b2.close()
+            del b2
+            torch.cuda.empty_cache()
+        line["all_configs"] = allc
+
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         cores = len(os.sched_getaffinity(0))
         r1, dt1 = oracle_rate(w, xy, off, n_events, cores, 1)
-        reps = max(1, min(50, int(12.0 / max(1e-3, dt1 * cores))))
+        reps = max(1, min(50, int(12.0 / max(1e-3, dt1))))
         rN, dtN = oracle_rate(w, xy, off, n_events, cores, reps)
         rS, dtS = oracle_rate(w, xy, off, min(n_events, 250), 1, 1)
         line["cpu_baseline"] = {"value": rN, "unit": UNIT, "cores": cores, "kind": "oracle",
                                 "sample": "the whole %d-event batch x %d passes, %d threads (%.1f s wall); single thread on the first %d events: %.0f events/s"
                                           % (n_events, reps, cores, dtN, min(n_events, 250), rS),
                                 "single_thread_value": rS}
-    h.close()
     if rank == 0:
         print(json.dumps(line), flush=True)
     if world > 1:

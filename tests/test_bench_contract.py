@@ -47,9 +47,18 @@ def test_gpu_arm_fails_loudly_without_a_gpu():
     assert "no CPU fallback" in (r.stderr + r.stdout)
 
 
-def test_traffic_table_is_readable():
+def test_default_arguments_and_blocks_of_the_gpu_arm():
     sys.path.insert(0, ROOT)
     import bench
-    t = bench.dram_traffic("cfg1_nominal")
-    assert isinstance(t, int) and t > 6_000_000          # at least the 6.16 MB of input
-    assert bench.dram_traffic("no such workload") is None
+    old = sys.argv
+    try:
+        sys.argv = ["bench.py"]
+        a = bench.parse_args()
+    finally:
+        sys.argv = old
+    assert a.gpus == 1 and a.config == 1 and a.warmup >= 3 and a.impl == "ours" and a.config_steps >= 20
+    assert not a.no_all_configs and a.sweep_events == 100000
+    src = open(os.path.join(ROOT, "bench.py")).read()
+    for key in ('"roofline"', '"cpu_baseline"', '"e2e"', '"all_configs"', '"multi_stream"', '"gpu_launches"', '"clocks"'):
+        assert key in src, key
+    assert "_work" not in src and "/root/reference" not in src

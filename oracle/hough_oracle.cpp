@@ -252,4 +252,12 @@ int oracle_rho_bin(float u, float v, float c, float s, float rho_max, int n_rho)
     return rho_bin(u, v, c, s, p);
 }
 
+// S3 + S4 alone, on a caller-made accumulator A [n_theta][n_rho] (so that a pin can hand-craft plateaus and borders
+// and check find_peaks itself).  Returns n_peaks (untruncated); peaks_out [max_peaks][3].
+int oracle_find_peaks(const uint32_t* A, int n_theta, int n_rho, int threshold, int max_peaks, uint32_t* peaks_out) {
+    Params p{};
+    p.n_theta = n_theta; p.n_rho = n_rho; p.threshold = threshold; p.max_peaks = max_peaks;
+    return find_peaks(A, p, peaks_out);
+}
+
 }  // extern "C"

@@ -53,10 +53,20 @@ typedef struct hough_peak {
     uint32_t votes;
 } hough_peak;
 
+/* Candidate circle and track parameters of one stored peak (hough_circles; Eq. (2)). 48 bytes.
+ * Lengths in the units of the hit coordinates; pt in GeV/c when those are mm and the field is in tesla. */
+typedef struct hough_circle {
+    double x_c, y_c, r_c;   /* centre and radius of the circle through the origin */
+    double pt;              /* 0.3 B r_c */
+    double phi0;            /* direction of motion at the origin, [0, 2 pi) */
+    int32_t charge;         /* +1 / -1 turning sense from the associated hits, 0 when undecided */
+    int32_t n_hits;         /* hits associated with the peak */
+} hough_circle;
+
 typedef enum hough_status {
     HOUGH_OK = 0,
     HOUGH_ERR_INVALID_ARG = -1,   /* null pointer, out-of-range value */
-    HOUGH_ERR_UNSUPPORTED = -2,   /* grid does not fit even an 8-CTA cluster's shared memory */
+    HOUGH_ERR_UNSUPPORTED = -2,   /* grid does not fit even a 16-CTA cluster's shared memory, or an option needs one CTA per event */
     HOUGH_ERR_CUDA = -3,          /* a CUDA call failed (no device, launch error, ...) */
     HOUGH_ERR_NOMEM = -4          /* host or device allocation failed */
 } hough_status;
@@ -65,11 +75,32 @@ typedef enum hough_option {
     HOUGH_OPT_MAX_PEAKS = 1,        /* peaks stored per event, 0..1048576 (default 64) */
     HOUGH_OPT_ACC_DTYPE = 2,        /* HOUGH_ACC_AUTO (= u16), HOUGH_ACC_U16, HOUGH_ACC_U32 */
     HOUGH_OPT_CONFORMAL_SCALE = 3,  /* 1 (Eq. (1) as printed, default) or 2 (the scale Eq. (2) implies) */
-    HOUGH_OPT_CLUSTER_SIZE = 4,     /* 0 = smallest of {1,2,4,8} that fits (default), else force 1,2,4,8 */
+    HOUGH_OPT_CLUSTER_SIZE = 4,     /* 0 = smallest of {1,2,4,8,16} that fits (default), else force one of them; 16 is a
+                                       non-portable cluster size, taken only when nothing smaller fits (the paper's own
+                                       1000 x 1000 grid) */
     HOUGH_OPT_CTAS_PER_SM = 5,      /* 0 = as many as fit, up to 2 (default); tuning knob */
-    HOUGH_OPT_VOTE_PATH = 6         /* 0 = fast voting with packed fp32x2 arithmetic, the exact slow path only for
+    HOUGH_OPT_VOTE_PATH = 6,        /* 0 = fast voting with packed fp32x2 arithmetic, the exact slow path only for
                                        degenerate hits (default); 1 = force the exact slow path everywhere (testing) */
+    /* Variants of the paper's own wording (readings Q18-Q20).  Any non-default
+       value selects the extended instantiation of the kernel; the defaults run the instantiation bench.py times. */
+    HOUGH_OPT_PEAK_MODE = 7,        /* 0 = absolute threshold + 3x3 local maximum, raster order (default);
+                                       1 = threshold relative to the event's global accumulator maximum + iterative
+                                       "extract the most significant peak, suppress its neighbourhood":
+                                       peaks come out in extraction order; needs one CTA per event */
+    HOUGH_OPT_REL_THRESHOLD_PERMILLE = 8,  /* peak mode 1: candidates need votes >= ceil(value * A_max / 1000) and >= threshold;
+                                       0..1000, default 500 */
+    HOUGH_OPT_NMS_RADIUS = 9,       /* peak mode 1: half-width in bins of the suppressed neighbourhood, 0..64 (default 1) */
+    HOUGH_OPT_THETA_WRAP = 10,      /* 1 = (theta + pi, rho) == (theta, -rho): column -1 is column n_theta-1 with the rho
+                                       index mirrored, for the 3x3 test, the suppression and the keep windows (default 0) */
+    HOUGH_OPT_KEEP_MODE = 11        /* 0 = (theta, rho) window around the stored peaks (default); 1 = original-space road
+                                       | ||hit - centre|| - r_c | < HOUGH_OPTF_KEEP_TOL around their candidate circles
+                                       ("inversely mapped back to the original space ... data filtering") */
 } hough_option;
+
+typedef enum hough_option_f64 {
+    HOUGH_OPTF_KEEP_TOL = 1,        /* keep mode 1: road half-width, units of the hit coordinates, >= 0 (default 0) */
+    HOUGH_OPTF_B_FIELD_TESLA = 2    /* hough_circles: magnetic field for pt = 0.3 B r_c (default 1.0) */
+} hough_option_f64;
 
 enum { HOUGH_ACC_AUTO = 0, HOUGH_ACC_U16 = 1, HOUGH_ACC_U32 = 2 };
 
@@ -99,6 +130,9 @@ hough_ctx* hough_create(int n_theta, int n_rho, float rho_max, int threshold, in
  * the handle is in flight.  HOUGH_ERR_UNSUPPORTED if the resulting
  * configuration does not fit the device. */
 int hough_set_option(hough_ctx* ctx, int key, long long value);
+
+/* Sets a real-valued option (see hough_option_f64). */
+int hough_set_option_f64(hough_ctx* ctx, int key, double value);
 
 /* Replaces the theta table of the rho matrix R ("discrete
  * angle theta_j", the cos/sin factors of PAPER.md:69): h_cos[j], h_sin[j],
@@ -148,6 +182,22 @@ typedef struct hough_io {
 } hough_io;
 
 int hough_run_ex(hough_ctx* ctx, const hough_io* io, hough_stream stream);
+
+/* Candidate-circle and track-parameter extraction for the stored peaks of a finished hough_run on the same
+ * stream: "the line in conformal space can be inversely mapped to the circular-track
+ * parameters" (Eq. (2) at :77), pT and phi0 as evaluated at PAPER.md:150-158.  Per stored peak
+ * (theta_j, rho bin k), in fp64 with one rounding per operation (readings Q14-Q17):
+ *   rho_c = (k + 0.5)/inv - rho_max (bin centre);  centre = s (cos theta_j, sin theta_j) / (2 rho_c);
+ *   r_c = s / (2 |rho_c|), s = the conformal scale (s = 2 is Eq. (2) as printed);  pt = 0.0003 B r_c;
+ *   a hit is associated with the peak iff its own bin at column j is within the keep window of k; the side of the
+ *   centre direction on which the associated hits lie gives the turning sense (charge) and
+ *   phi0 = centre azimuth - charge * pi/2.
+ *   d_peaks, d_counts  as written by hough_run for the same d_xy / d_event_offsets
+ *   d_circles          [n_events][max_peaks] hough_circle; the first min(n_peaks, max_peaks) entries of an event are
+ *                      written, the rest are untouched
+ * One kernel launch, asynchronous on `stream`, no allocation, capturable. */
+int hough_circles(hough_ctx* ctx, const float* d_xy, const int32_t* d_event_offsets, int n_events,
+                  const hough_peak* d_peaks, const int32_t* d_counts, hough_circle* d_circles, hough_stream stream);
 
 /* End-to-end form with HOST buffers (pinned memory recommended), the shape of
  * the paper's own measurement: events are "transmitted to the GPU memory" in

@@ -14,13 +14,13 @@ extern "C" {
  * device with `smem_optin` bytes of opt-in shared memory per CTA (0 = B200's 232448).  Needs NO CUDA device.
  * Writes HOUGH_PLAN_N_FIELDS values to out[] in the order of enum hough_plan_field; n_out must be at least
  * that.  Returns 0, HOUGH_ERR_INVALID_ARG, or HOUGH_ERR_UNSUPPORTED if nothing fits. */
-enum { HOUGH_PLAN_N_FIELDS = 26 };
+enum { HOUGH_PLAN_N_FIELDS = 27 };
 typedef enum hough_plan_field {
     HOUGH_PLAN_CLUSTER_SIZE = 0, HOUGH_PLAN_THREADS, HOUGH_PLAN_SMEM_BYTES, HOUGH_PLAN_ACC_BITS, HOUGH_PLAN_COLS_PER_LANE,
     HOUGH_PLAN_COLS_PER_CTA, HOUGH_PLAN_N_GROUPS, HOUGH_PLAN_N_STRIPES, HOUGH_PLAN_PITCH_BYTES, HOUGH_PLAN_BITMAP_WORDS_PER_ROW,
     HOUGH_PLAN_CHUNK_HITS, HOUGH_PLAN_REGION_BYTES, HOUGH_PLAN_PBM_OFF, HOUGH_PLAN_PBM_BYTES, HOUGH_PLAN_HB_OFF, HOUGH_PLAN_MISC_OFF,
     HOUGH_PLAN_W8_OFF, HOUGH_PLAN_W8_PITCH, HOUGH_PLAN_MCF_OFF, HOUGH_PLAN_MSF_OFF, HOUGH_PLAN_COLQ_OFF, HOUGH_PLAN_STASH_OFF,
-    HOUGH_PLAN_CNT_OFF, HOUGH_PLAN_GCNT_OFF, HOUGH_PLAN_RCP_GROUPS, HOUGH_PLAN_RCP_2S
+    HOUGH_PLAN_CNT_OFF, HOUGH_PLAN_GCNT_OFF, HOUGH_PLAN_RCP_GROUPS, HOUGH_PLAN_RCP_2S, HOUGH_PLAN_CIRC_CAP
 } hough_plan_field;
 int hough_plan_describe(int n_theta, int n_rho, int acc_dtype, int cluster_size, int ctas_per_sm, int smem_optin,
                         long long* out, int n_out);

@@ -23,6 +23,13 @@ HOUGH_OPT_CONFORMAL_SCALE = 3
 HOUGH_OPT_CLUSTER_SIZE = 4
 HOUGH_OPT_CTAS_PER_SM = 5
 HOUGH_OPT_VOTE_PATH = 6
+HOUGH_OPT_PEAK_MODE = 7
+HOUGH_OPT_REL_THRESHOLD_PERMILLE = 8
+HOUGH_OPT_NMS_RADIUS = 9
+HOUGH_OPT_THETA_WRAP = 10
+HOUGH_OPT_KEEP_MODE = 11
+HOUGH_OPTF_KEEP_TOL = 1
+HOUGH_OPTF_B_FIELD_TESLA = 2
 HOUGH_ACC_AUTO, HOUGH_ACC_U16, HOUGH_ACC_U32 = 0, 1, 2
 
 HOUGH_INFO_CLUSTER_SIZE = 1
@@ -38,8 +45,8 @@ HOUGH_INFO_LAUNCHES = 10
 
 # what each header under include/ declares, and which library exports it
 EXPORTS = [            # include/hough.h -> libhough_b200.so (the product ABI)
-    "hough_create", "hough_set_option", "hough_set_trig_table", "hough_get_info", "hough_run", "hough_run_ex",
-    "hough_run_host", "hough_destroy", "hough_strerror", "hough_last_error", "hough_version",
+    "hough_create", "hough_set_option", "hough_set_option_f64", "hough_set_trig_table", "hough_get_info", "hough_run", "hough_run_ex",
+    "hough_circles", "hough_run_host", "hough_destroy", "hough_strerror", "hough_last_error", "hough_version",
 ]
 DEBUG_EXPORTS = ["hough_plan_describe", "hough_debug_tame_bounds", "hough_debug_bounds_enabled"]   # include/hough_debug.h, same library
 BENCH_EXPORTS = ["hough_bench_shared_atomics", "hough_bench_vote_loop", "hough_bench_issue_rate"]   # include/hough_bench.h -> libhough_bench.so
@@ -86,6 +93,10 @@ def load_library():
     lib.hough_create.argtypes = [ci, ci, ctypes.c_float, ci, ci]
     lib.hough_set_option.restype = ci
     lib.hough_set_option.argtypes = [vp, ci, cll]
+    lib.hough_set_option_f64.restype = ci
+    lib.hough_set_option_f64.argtypes = [vp, ci, ctypes.c_double]
+    lib.hough_circles.restype = ci
+    lib.hough_circles.argtypes = [vp, vp, vp, ci, vp, vp, vp, vp]
     lib.hough_set_trig_table.restype = ci
     lib.hough_set_trig_table.argtypes = [vp, vp, vp]
     lib.hough_get_info.restype = cll
@@ -175,6 +186,23 @@ def hough_set_option(ctx, key, value):
     _check(load_library().hough_set_option(ctx, key, value), "hough_set_option")
 
 
+def hough_set_option_f64(ctx, key, value):
+    _check(load_library().hough_set_option_f64(ctx, key, float(value)), "hough_set_option_f64")
+
+
+def hough_circles(ctx, d_xy, d_event_offsets, n_events, d_peaks, d_counts, d_circles, stream=None):
+    """d_circles: CUDA uint8 tensor of at least n_events * max_peaks * 48 bytes (hough_circle records)."""
+    import torch
+    mp = hough_get_info(ctx, HOUGH_INFO_MAX_PEAKS)
+    _marshal_check(True, n_events, d_xy, d_event_offsets, None, d_peaks, d_counts, max_peaks=mp)
+    if n_events > 0 and mp > 0:
+        if not (isinstance(d_circles, torch.Tensor) and d_circles.is_cuda and d_circles.is_contiguous() and d_circles.dtype == torch.uint8
+                and d_circles.numel() >= 48 * n_events * mp):
+            raise HoughError("d_circles must be a contiguous CUDA uint8 tensor of at least n_events * max_peaks * 48 bytes")
+    _check(load_library().hough_circles(ctx, _ptr(d_xy), _ptr(d_event_offsets), n_events, _ptr(d_peaks), _ptr(d_counts),
+                                        _ptr(d_circles), _stream_handle(stream)), "hough_circles")
+
+
 def hough_set_trig_table(ctx, h_cos, h_sin):
     """h_cos, h_sin: contiguous float32 numpy arrays (HOST) of n_theta entries."""
     import numpy as np
@@ -212,7 +240,7 @@ def _marshal_check(cuda, n_events, xy, off, keep, peaks, counts, kept_xy=None, k
         return                         # the C ABI reports the null pointer
     n_total = xy.numel() // 2
     chk("xy", xy, torch.float32, 0)
-    chk("keep mask", keep, torch.uint8, n_total)
+    chk("keep mask", keep, torch.uint8, n_total)     # None (hough_circles) is skipped
     chk("counts", counts, torch.int32, 2 * n_events)
     if max_peaks:
         chk("peaks", peaks, torch.int32, 2 * n_events * max_peaks)
@@ -298,7 +326,7 @@ def hough_debug_bounds_enabled():
 
 PLAN_FIELDS = ("cluster_size", "threads", "smem_bytes", "acc_bits", "cols_per_lane", "cols_per_cta", "n_groups", "n_stripes",
                "pitch_bytes", "bitmap_words_per_row", "chunk_hits", "region_bytes", "pbm_off", "pbm_bytes", "hb_off", "misc_off",
-               "w8_off", "w8_pitch", "mcf_off", "msf_off", "colq_off", "stash_off", "cnt_off", "gcnt_off", "rcp_groups", "rcp_2s")
+               "w8_off", "w8_pitch", "mcf_off", "msf_off", "colq_off", "stash_off", "cnt_off", "gcnt_off", "rcp_groups", "rcp_2s", "circ_cap")
 
 
 def hough_plan_describe(n_theta, n_rho, acc_dtype=HOUGH_ACC_AUTO, cluster_size=0, ctas_per_sm=0, smem_optin=0):
@@ -314,7 +342,8 @@ class Hough:
     """Owns a hough_ctx and allocates output tensors.  No arithmetic of the method happens here."""
 
     def __init__(self, n_theta, n_rho, rho_max, threshold, window, max_peaks=64, acc_dtype="u16",
-                 conformal_scale=1, cluster_size=0, ctas_per_sm=0, trig_table=None):
+                 conformal_scale=1, cluster_size=0, ctas_per_sm=0, trig_table=None, peak_mode=0, rel_permille=500,
+                 nms_radius=1, theta_wrap=False, keep_mode=0, keep_tol=0.0, b_field=1.0):
         self.n_theta, self.n_rho, self.max_peaks = n_theta, n_rho, max_peaks
         self.ctx = hough_create(n_theta, n_rho, float(rho_max), threshold, window)
         try:
@@ -328,6 +357,17 @@ class Hough:
                 hough_set_option(self.ctx, HOUGH_OPT_CTAS_PER_SM, ctas_per_sm)
             if trig_table is not None:
                 hough_set_trig_table(self.ctx, trig_table[0], trig_table[1])
+            if peak_mode:
+                hough_set_option(self.ctx, HOUGH_OPT_PEAK_MODE, peak_mode)
+                hough_set_option(self.ctx, HOUGH_OPT_REL_THRESHOLD_PERMILLE, rel_permille)
+                hough_set_option(self.ctx, HOUGH_OPT_NMS_RADIUS, nms_radius)
+            if theta_wrap:
+                hough_set_option(self.ctx, HOUGH_OPT_THETA_WRAP, 1)
+            if keep_mode:
+                hough_set_option(self.ctx, HOUGH_OPT_KEEP_MODE, keep_mode)
+                hough_set_option_f64(self.ctx, HOUGH_OPTF_KEEP_TOL, keep_tol)
+            if b_field != 1.0:
+                hough_set_option_f64(self.ctx, HOUGH_OPTF_B_FIELD_TESLA, b_field)
         except Exception:
             self.close()
             raise
@@ -360,6 +400,15 @@ class Hough:
                      out.get("kept_xy"), out.get("kept_idx"), out.get("accum"), stream)
         return out
 
+    def circles(self, d_xy, d_offsets, out, stream=None):
+        """Candidate circles of the stored peaks of `out` (the dict run() returned): a CUDA uint8 tensor
+        [n_events, max_peaks, 48] of hough_circle records (view it with CIRCLE_DTYPE on the host)."""
+        import torch
+        n_events = d_offsets.numel() - 1
+        circ = torch.zeros((n_events, max(self.max_peaks, 1), 48), dtype=torch.uint8, device=d_xy.device)[:, :self.max_peaks]
+        hough_circles(self.ctx, d_xy, d_offsets, n_events, out["peaks"], out["counts"], circ, stream)
+        return circ
+
     def close(self):
         if getattr(self, "ctx", None):
             hough_destroy(self.ctx)
@@ -370,6 +419,12 @@ class Hough:
             self.close()
         except Exception:
             pass
+
+
+def circle_dtype():
+    """numpy dtype of hough_circle (include/hough.h): pure layout, for viewing the bytes hough_circles wrote."""
+    import numpy as np
+    return np.dtype([("x_c", "<f8"), ("y_c", "<f8"), ("r_c", "<f8"), ("pt", "<f8"), ("phi0", "<f8"), ("charge", "<i4"), ("n_hits", "<i4")])
 
 
 def unpack_peaks(peaks_i32):

@@ -60,6 +60,8 @@ struct hough_ctx {
     int opt_cluster = 0;
     int opt_ctas_per_sm = 0;
     int opt_vote_path = 0;
+    int peak_mode = 0, rel_permille = 500, nms_radius = 1, theta_wrap = 0, keep_mode = 0;
+    double keep_tol = 0.0, b_field = 1.0;
     int device = 0;
     int sm_count = 0;
     int smem_optin = 0;
@@ -84,19 +86,27 @@ struct hough_ctx {
 
 namespace {
 
-template <bool ACC16, bool CL>
+template <bool ACC16, bool CL, bool EXT>
 const void* kernel_ptr(int cpl) {
     switch (cpl) {
-        case 6: return (const void*)&hough::hough_event_kernel<ACC16, CL, 6>;
-        case 4: return (const void*)&hough::hough_event_kernel<ACC16, CL, 4>;
-        default: return (const void*)&hough::hough_event_kernel<ACC16, CL, 2>;
+        case 6: return (const void*)&hough::hough_event_kernel<ACC16, CL, 6, EXT>;
+        case 4: return (const void*)&hough::hough_event_kernel<ACC16, CL, 4, EXT>;
+        default: return (const void*)&hough::hough_event_kernel<ACC16, CL, 2, EXT>;
     }
 }
 
-const void* pick_kernel(bool acc16, bool cl, int cpl) {
-    if (acc16) return cl ? kernel_ptr<true, true>(cpl) : kernel_ptr<true, false>(cpl);
-    return cl ? kernel_ptr<false, true>(cpl) : kernel_ptr<false, false>(cpl);
+// ext: the extended instantiation (peak mode, theta wrap, distance filter); the default options never take it, so the
+// kernel bench.py times is compiled without any of that code.
+const void* pick_kernel(bool acc16, bool cl, int cpl, bool ext) {
+    if (ext) {
+        if (acc16) return cl ? kernel_ptr<true, true, true>(cpl) : kernel_ptr<true, false, true>(cpl);
+        return cl ? kernel_ptr<false, true, true>(cpl) : kernel_ptr<false, false, true>(cpl);
+    }
+    if (acc16) return cl ? kernel_ptr<true, true, false>(cpl) : kernel_ptr<true, false, false>(cpl);
+    return cl ? kernel_ptr<false, true, false>(cpl) : kernel_ptr<false, false, false>(cpl);
 }
+
+bool wants_ext(const hough_ctx* c) { return c->peak_mode != 0 || c->theta_wrap != 0 || c->keep_mode != 0; }
 
 // cudaFuncAttributeMaxDynamicSharedMemorySize belongs to the kernel (per device), not to a handle: several live
 // handles may share one instantiation with different footprints, so the attribute is only ever RAISED.
@@ -108,6 +118,14 @@ int raise_smem_limit(int device, const void* fn, int bytes) {
     if (bytes <= h) return HOUGH_OK;
     CUDA_TRY(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
     h = bytes;
+    return HOUGH_OK;
+}
+
+// Launch attributes of the kernel this handle would launch now: shared-memory limit (raised, never lowered) and, for a
+// 16-CTA cluster, the non-portable-cluster-size permission.
+int prepare_kernel(int device, const void* fn, int smem_bytes, int csize) {
+    if (int rc = raise_smem_limit(device, fn, smem_bytes)) return rc;
+    if (csize > 8) CUDA_TRY(cudaFuncSetAttribute(fn, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
     return HOUGH_OK;
 }
 
@@ -148,8 +166,10 @@ bool try_plan(const hough_ctx* c, bool acc16, int C, int want_ctas, Plan* out) {
     kp.stash_off = (int)o;   o += (C > 1) ? align_up(HOUGH_SEL_ROUND_BLOCKS * nwarps * 4, 16) : 0;
     kp.cnt_off = (int)o;     o += (C > 1) ? align_up(HOUGH_SEL_ROUND_BLOCKS * 4, 16) : 0;
     kp.gcnt_off = (int)o;    o += (C > 1) ? align_up((HOUGH_SEL_ROUND_BLOCKS * C + 1) * 4, 16) : 0;
+    const long long post_bytes = o;
     const long long region = align_up((int)std::max(acc_bytes, o), 16);
-    const long long pbm_bytes = align_up(cols * wpr * 4, 16);
+    // the peak bitmap; iterative NMS (peak mode 1) keeps one 8-byte key per rho row there instead
+    const long long pbm_bytes = std::max(align_up(cols * wpr * 4, 16), align_up(8 * c->n_rho, 16));
     const long long misc_bytes = 256;
     const long long fixed = region + pbm_bytes + misc_bytes;
     // per-CTA budget: the SM has 228 KB, each resident CTA reserves 1 KB; a single CTA may opt in to smem_optin
@@ -177,6 +197,10 @@ bool try_plan(const hough_ctx* c, bool acc16, int C, int want_ctas, Plan* out) {
     kp.pbm_off = (int)region;
     kp.pbm_bytes = (int)pbm_bytes;
     kp.hb_off = (int)(region + pbm_bytes);
+    // distance filter: (x_c, y_c, r_c) doubles staged from the start of the dead accumulator region, in a cluster up to
+    // the compaction scratch (stash/cnt/gcnt live there at the same time)
+    kp.circ_cap = (int)(((C > 1 ? (long long)kp.stash_off : region) - kp.w8_off) / 24);
+    (void)post_bytes;
     kp.misc_off = kp.hb_off + (int)chunk * 8;
     out->acc16 = acc16;
     out->cpl = cpl;
@@ -190,8 +214,8 @@ bool try_plan(const hough_ctx* c, bool acc16, int C, int want_ctas, Plan* out) {
 // Pure host logic (no CUDA call): the smallest cluster of {1,2,4,8} CTAs whose layout fits, two CTAs per SM if possible.
 bool choose_plan(const hough_ctx* c, Plan* best) {
     const bool acc16 = c->acc_dtype != HOUGH_ACC_U32;
-    const int cands[4] = {1, 2, 4, 8};
-    for (int ci = 0; ci < 4; ++ci) {
+    const int cands[5] = {1, 2, 4, 8, 16};   // 16 = non-portable cluster size, only when nothing smaller fits
+    for (int ci = 0; ci < 5; ++ci) {
         const int C = cands[ci];
         if (c->opt_cluster && C != c->opt_cluster) continue;
         if (C > c->n_theta) continue;
@@ -209,12 +233,12 @@ int make_plan(hough_ctx* c) {
     if (!choose_plan(c, &best))
         return fail(HOUGH_ERR_UNSUPPORTED, "a %d x %d %s accumulator does not fit the shared memory of %s",
                     c->n_theta, c->n_rho, acc16 ? "u16" : "u32",
-                    c->opt_cluster ? "the requested cluster size" : "an 8-CTA cluster");
-    const void* fn = pick_kernel(best.acc16, best.csize > 1, best.cpl);
+                    c->opt_cluster ? "the requested cluster size" : "a 16-CTA cluster");
+    const void* fn = pick_kernel(best.acc16, best.csize > 1, best.cpl, false);
     int cur = -1;
     CUDA_TRY(cudaGetDevice(&cur));
     if (cur != c->device) return fail(HOUGH_ERR_INVALID_ARG, "the handle belongs to device %d but device %d is current", c->device, cur);
-    if (int rc = raise_smem_limit(c->device, fn, best.smem_bytes)) return rc;
+    if (int rc = prepare_kernel(c->device, fn, best.smem_bytes, best.csize)) return rc;
     int occ = 0;
     if (best.csize == 1) {
         CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fn, best.threads, best.smem_bytes));
@@ -232,8 +256,11 @@ int make_plan(hough_ctx* c) {
         at.val.clusterDim.x = (unsigned)best.csize; at.val.clusterDim.y = 1; at.val.clusterDim.z = 1;
         cfg.attrs = &at; cfg.numAttrs = 1;
         int ncl = 0;
-        CUDA_TRY(cudaOccupancyMaxActiveClusters(&ncl, fn, &cfg));
-        if (ncl < 1) return fail(HOUGH_ERR_UNSUPPORTED, "no %d-CTA cluster of this kernel fits the device", best.csize);
+        const cudaError_t oe = cudaOccupancyMaxActiveClusters(&ncl, fn, &cfg);
+        if (oe != cudaSuccess) (void)cudaGetLastError();
+        if (oe != cudaSuccess || ncl < 1)
+            return fail(HOUGH_ERR_UNSUPPORTED, "no %d-CTA cluster of this kernel fits the device (%s)", best.csize,
+                        oe != cudaSuccess ? cudaGetErrorString(oe) : "0 active clusters");
         best.grid_max = ncl * best.csize;
         best.ctas_per_sm = (best.grid_max + c->sm_count - 1) / c->sm_count;
     }
@@ -303,6 +330,11 @@ int launch(hough_ctx* c, const hough_io* io, cudaStream_t stream) {
 #ifdef HOUGH_DIAG
     kp.diag = c->opt_vote_path >= 2 ? c->opt_vote_path : 0;
 #endif
+    const bool ext = wants_ext(c);
+    if (ext && c->peak_mode == 1 && pl.csize > 1)
+        return fail(HOUGH_ERR_UNSUPPORTED, "peak mode 1 (iterative NMS) needs the accumulator in one CTA; this grid takes a %d-CTA cluster", pl.csize);
+    kp.peak_mode = c->peak_mode; kp.rel_permille = c->rel_permille; kp.nms_radius = c->nms_radius;
+    kp.theta_wrap = c->theta_wrap; kp.keep_mode = c->keep_mode; kp.keep_tol = c->keep_tol;
     const int C = pl.csize;
     // one CTA (cluster) per event: the hardware block scheduler deals events to the SM slots as they free up, which
     // balances events of different size; the kernel's event loop only matters beyond 2^31 CTAs
@@ -310,7 +342,9 @@ int launch(hough_ctx* c, const hough_io* io, cudaStream_t stream) {
     int grid = (int)std::min<long long>(want, 0x7FFFFFF0LL);
     grid = grid / C * C;
     if (grid < C) grid = C;
-    const void* fn = pick_kernel(pl.acc16, C > 1, pl.cpl);
+    const void* fn = pick_kernel(pl.acc16, C > 1, pl.cpl, ext);
+    if (ext)   // the extended instantiation is a different kernel: its attributes are set on first use (cheap afterwards)
+        if (int rc = prepare_kernel(c->device, fn, pl.smem_bytes, C)) return rc;
     cudaLaunchConfig_t cfg{};
     cfg.gridDim = dim3((unsigned)grid);
     cfg.blockDim = dim3((unsigned)pl.threads);
@@ -379,6 +413,24 @@ int hough_set_option(hough_ctx* c, int key, long long value) {
     if (!c) return fail(HOUGH_ERR_INVALID_ARG, "null handle");
     const int o_mp = c->max_peaks, o_acc = c->acc_dtype, o_sc = c->conformal_scale, o_cl = c->opt_cluster,
               o_cps = c->opt_ctas_per_sm, o_vp = c->opt_vote_path;
+    switch (key) {   // options that need no new plan
+        case HOUGH_OPT_PEAK_MODE:
+            if (value != 0 && value != 1) return fail(HOUGH_ERR_INVALID_ARG, "peak mode must be 0 or 1");
+            c->peak_mode = (int)value; return HOUGH_OK;
+        case HOUGH_OPT_REL_THRESHOLD_PERMILLE:
+            if (value < 0 || value > 1000) return fail(HOUGH_ERR_INVALID_ARG, "relative threshold must be 0..1000 permille");
+            c->rel_permille = (int)value; return HOUGH_OK;
+        case HOUGH_OPT_NMS_RADIUS:
+            if (value < 0 || value > 64) return fail(HOUGH_ERR_INVALID_ARG, "NMS radius must be 0..64");
+            c->nms_radius = (int)value; return HOUGH_OK;
+        case HOUGH_OPT_THETA_WRAP:
+            if (value != 0 && value != 1) return fail(HOUGH_ERR_INVALID_ARG, "theta wrap must be 0 or 1");
+            c->theta_wrap = (int)value; return HOUGH_OK;
+        case HOUGH_OPT_KEEP_MODE:
+            if (value != 0 && value != 1) return fail(HOUGH_ERR_INVALID_ARG, "keep mode must be 0 or 1");
+            c->keep_mode = (int)value; return HOUGH_OK;
+        default: break;
+    }
     switch (key) {
         case HOUGH_OPT_MAX_PEAKS:
             if (value < 0 || value > 1048576) return fail(HOUGH_ERR_INVALID_ARG, "max_peaks must be in 0..1048576");
@@ -390,7 +442,8 @@ int hough_set_option(hough_ctx* c, int key, long long value) {
             if (value != 1 && value != 2) return fail(HOUGH_ERR_INVALID_ARG, "conformal scale must be 1 or 2");
             c->conformal_scale = (int)value; return HOUGH_OK;
         case HOUGH_OPT_CLUSTER_SIZE:
-            if (value != 0 && value != 1 && value != 2 && value != 4 && value != 8) return fail(HOUGH_ERR_INVALID_ARG, "cluster size must be 0,1,2,4,8");
+            if (value != 0 && value != 1 && value != 2 && value != 4 && value != 8 && value != 16)
+                return fail(HOUGH_ERR_INVALID_ARG, "cluster size must be 0,1,2,4,8,16");
             c->opt_cluster = (int)value; break;
         case HOUGH_OPT_CTAS_PER_SM:
             if (value < 0 || value > 2) return fail(HOUGH_ERR_INVALID_ARG, "ctas_per_sm must be 0,1,2");
@@ -411,6 +464,41 @@ int hough_set_option(hough_ctx* c, int key, long long value) {
         c->opt_ctas_per_sm = o_cps; c->opt_vote_path = o_vp;
     }
     return rc;
+}
+
+int hough_set_option_f64(hough_ctx* c, int key, double value) {
+    if (!c) return fail(HOUGH_ERR_INVALID_ARG, "null handle");
+    switch (key) {
+        case HOUGH_OPTF_KEEP_TOL:
+            if (!(value >= 0.0)) return fail(HOUGH_ERR_INVALID_ARG, "the keep tolerance must be >= 0");
+            c->keep_tol = value; return HOUGH_OK;
+        case HOUGH_OPTF_B_FIELD_TESLA:
+            if (!std::isfinite(value)) return fail(HOUGH_ERR_INVALID_ARG, "the field must be finite");
+            c->b_field = value; return HOUGH_OK;
+        default:
+            return fail(HOUGH_ERR_INVALID_ARG, "unknown real-valued option %d", key);
+    }
+}
+
+int hough_circles(hough_ctx* c, const float* d_xy, const int32_t* d_event_offsets, int n_events, const hough_peak* d_peaks,
+                  const int32_t* d_counts, hough_circle* d_circles, hough_stream stream) {
+    if (!c) return fail(HOUGH_ERR_INVALID_ARG, "null handle");
+    if (n_events < 0) return fail(HOUGH_ERR_INVALID_ARG, "n_events < 0");
+    if (n_events == 0 || c->max_peaks == 0) return HOUGH_OK;
+    if (!d_xy || !d_event_offsets || !d_peaks || !d_counts || !d_circles) return fail(HOUGH_ERR_INVALID_ARG, "null device pointer");
+    int cur = -1;
+    if (cudaGetDevice(&cur) != cudaSuccess || cur != c->device)
+        return fail(HOUGH_ERR_INVALID_ARG, "the handle belongs to device %d but device %d is current", c->device, cur);
+    hough::CParams cp{};
+    cp.xy = (const float2*)d_xy; cp.off = d_event_offsets; cp.n_events = n_events; cp.peaks = d_peaks; cp.counts = d_counts;
+    cp.out = d_circles; cp.cos_t = c->d_cos; cp.sin_t = c->d_sin;
+    cp.n_theta = c->n_theta; cp.n_rho = c->n_rho; cp.window = c->window; cp.max_peaks = c->max_peaks;
+    cp.rho_max = c->rho_max; cp.inv = c->inv; cp.scale = (float)c->conformal_scale; cp.b_field = c->b_field;
+    const int grid = (int)std::min<long long>(n_events, 0x7FFFFFF0LL);
+    void* args[1] = {(void*)&cp};
+    CUDA_TRY(cudaLaunchKernel((const void*)&hough::hough_circles_kernel, dim3((unsigned)grid), dim3(256), args, 0, (cudaStream_t)stream));
+    c->launches.fetch_add(1);
+    return HOUGH_OK;
 }
 
 int hough_set_trig_table(hough_ctx* c, const float* h_cos, const float* h_sin) {
@@ -531,8 +619,8 @@ int hough_plan_describe(int n_theta, int n_rho, int acc_dtype, int cluster_size,
     if (n_theta < 1 || n_theta > 65535 || n_rho < 1 || n_rho > 65535 || !out || n_out < HOUGH_PLAN_N_FIELDS)
         return fail(HOUGH_ERR_INVALID_ARG, "bad argument");
     if (acc_dtype != HOUGH_ACC_AUTO && acc_dtype != HOUGH_ACC_U16 && acc_dtype != HOUGH_ACC_U32) return fail(HOUGH_ERR_INVALID_ARG, "bad accumulator dtype");
-    if (cluster_size != 0 && cluster_size != 1 && cluster_size != 2 && cluster_size != 4 && cluster_size != 8)
-        return fail(HOUGH_ERR_INVALID_ARG, "cluster size must be 0,1,2,4,8");
+    if (cluster_size != 0 && cluster_size != 1 && cluster_size != 2 && cluster_size != 4 && cluster_size != 8 && cluster_size != 16)
+        return fail(HOUGH_ERR_INVALID_ARG, "cluster size must be 0,1,2,4,8,16");
     if (ctas_per_sm < 0 || ctas_per_sm > 2) return fail(HOUGH_ERR_INVALID_ARG, "ctas_per_sm must be 0,1,2");
     hough_ctx c;
     c.n_theta = n_theta; c.n_rho = n_rho; c.threshold = 1; c.window = 0; c.rho_max = 1.0f; c.inv = 1.0f;
@@ -544,7 +632,7 @@ int hough_plan_describe(int n_theta, int n_rho, int acc_dtype, int cluster_size,
     const long long v[HOUGH_PLAN_N_FIELDS] = {
         pl.csize, pl.threads, pl.smem_bytes, pl.acc16 ? 16 : 32, pl.cpl, k.cols_per_cta, k.n_groups, k.n_stripes,
         k.pitch_b, k.wpr, k.chunk, k.region_bytes, k.pbm_off, k.pbm_bytes, k.hb_off, k.misc_off,
-        k.w8_off, k.w8_pitch, k.mcf_off, k.msf_off, k.colq_off, k.stash_off, k.cnt_off, k.gcnt_off, k.rcp_groups, k.rcp_2s};
+        k.w8_off, k.w8_pitch, k.mcf_off, k.msf_off, k.colq_off, k.stash_off, k.cnt_off, k.gcnt_off, k.rcp_groups, k.rcp_2s, k.circ_cap};
     for (int i = 0; i < HOUGH_PLAN_N_FIELDS; ++i) out[i] = v[i];
     return HOUGH_OK;
 }

@@ -98,7 +98,29 @@ struct KParams {
     int misc_off;         // 64 ints
     // post-extraction layout inside the accumulator region (byte offsets)
     int w8_off, w8_pitch, mcf_off, msf_off, colq_off, stash_off, cnt_off, gcnt_off;
+    // options of the extended instantiation (EXT = true; readings Q18-Q20).
+    // The default instantiation (EXT = false) never reads them.
+    int peak_mode;        // 0: threshold + 3x3 local maximum; 1: relative threshold + iterative NMS
+    int rel_permille;     // NMS: candidates need a >= ceil(rel_permille * A_max / 1000) (and >= threshold)
+    int nms_radius;       // NMS: half-width of the suppressed neighbourhood
+    int theta_wrap;       // column -1 is column n_theta-1 with the rho index mirrored
+    int keep_mode;        // 0: (theta, rho) window; 1: distance to the candidate circle
+    int circ_cap;         // distance filter: circles staged in the dead accumulator region
+    double keep_tol;      // distance filter tolerance, units of the hit coordinates
 };
+
+// Candidate circle of a peak (Eq. (2), with the conformal scale s of reading Q1; DESIGN.md readings
+// Q14, Q15): rho_c = (k + 0.5) / inv - rho_max at the centre of the bin, centre = s (c_j, s_j) / (2 rho_c),
+// r_c = s / (2 |rho_c|); fp64, one rounding per operation (the TU is built with -fmad=false), IEEE division.
+__device__ __forceinline__ double rho_centre(int k, float inv, float rho_max) {
+    return __dsub_rn(__ddiv_rn(__dadd_rn((double)k, 0.5), (double)inv), (double)rho_max);
+}
+__device__ __forceinline__ void circle_of(float cj, float sj, int k, float inv, float rho_max, float scale, double& x_c, double& y_c, double& r_c) {
+    const double den = __dmul_rn(2.0, rho_centre(k, inv, rho_max)), s = (double)scale;
+    x_c = __ddiv_rn(__dmul_rn(s, (double)cj), den);
+    y_c = __ddiv_rn(__dmul_rn(s, (double)sj), den);
+    r_c = __ddiv_rn(s, fabs(den));
+}
 
 // ---------------------------------------------------------------- small helpers
 #ifdef HOUGH_HOST_EMU
@@ -232,7 +254,7 @@ __device__ __forceinline__ unsigned cell_from(const unsigned char* acc, int pitc
 }
 
 // ---------------------------------------------------------------- the kernel
-template <bool ACC16, bool CL, int CPL>
+template <bool ACC16, bool CL, int CPL, bool EXT = false>
 __global__ void __launch_bounds__(1024, 1) hough_event_kernel(const __grid_constant__ KParams p) {
     HOUGH_DYN_SMEM(smem);
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -399,6 +421,95 @@ __global__ void __launch_bounds__(1024, 1) hough_event_kernel(const __grid_const
             }
         }
 
+        int n_stored;
+        if (EXT && !CL && p.peak_mode == 1) {
+            // ---- N2: threshold relative to the global maximum + iterative "extract the most
+            // significant peak, suppress its neighbourhood" (reading Q18).  One CTA holds the whole
+            // accumulator.  rowkey[k] = best cell of rho row k as (votes << 32) | (0xFFFF - j) << 16 | (0xFFFF - k): the
+            // maximum over keys is the largest count and, among equals, the raster-first cell.  All warps build the row
+            // keys; warp 0 then runs the extraction loop alone (a few hundred cycles per peak: 2R+1 rows to refresh).
+            ull* rowkey = (ull*)pbm;      // the peak bitmap is unused in this mode; the planner sizes it for n_rho keys
+            auto warp_max = [&](ull best) -> ull {
+#pragma unroll
+                for (int d = 16; d >= 1; d >>= 1) {
+                    const ull o = __shfl_xor_sync(0xffffffffu, best, d);
+                    if (o > best) best = o;
+                }
+                return best;
+            };
+            auto row_best = [&](int k) -> ull {
+                ull best = 0;
+                for (int jl = lane; jl < ncols; jl += 32) {
+                    if (!HB_CHK((unsigned)k * pitch + 4u * cell_word_off<ACC16>(jl) + 4 <= limit, HB_H4)) continue;
+                    const unsigned a = cell_from<ACC16>(acc, p.pitch_b, jl, k);
+                    const ull key = ((ull)a << 32) | ((ull)(0xFFFFu - (unsigned)(col0 + jl)) << 16) | (ull)(0xFFFFu - (unsigned)k);
+                    if (a != 0u && key > best) best = key;
+                }
+                return warp_max(best);
+            };
+            for (int k = warp; k < p.n_rho; k += nwarps) {
+                const ull b = row_best(k);
+                if (lane == 0 && HB_CHK(8 * k + 8 <= p.pbm_bytes, HB_H4)) rowkey[k] = b;
+            }
+            __syncthreads();
+            if (warp == 0) {
+                auto global_best = [&]() -> ull {
+                    ull best = 0;
+                    for (int k = lane; k < p.n_rho; k += 32)
+                        if (HB_CHK(8 * k + 8 <= p.pbm_bytes, HB_H4)) { const ull b = rowkey[k]; if (b > best) best = b; }
+                    return warp_max(best);
+                };
+                ull best = global_best();
+                const ull rel = ((ull)p.rel_permille * (ull)(unsigned)(best >> 32) + 999ull) / 1000ull;
+                const ull thr_eff = (ull)p.threshold > rel ? (ull)p.threshold : rel;
+                const int R = p.nms_radius, side = 2 * R + 1;
+                int n_found = 0;
+                for (;;) {
+                    const unsigned a = (unsigned)(best >> 32);
+                    if (a == 0u || (ull)a < thr_eff) break;
+                    const int j = 0xFFFF - (int)((best >> 16) & 0xFFFFull), k = 0xFFFF - (int)(best & 0xFFFFull);
+                    if (lane == 0 && n_found < p.max_peaks) {
+                        hough_peak pk;
+                        pk.theta_bin = (uint16_t)j; pk.rho_bin = (uint16_t)k; pk.votes = a;
+                        p.peaks[(size_t)e * p.max_peaks + n_found] = pk;
+                    }
+                    ++n_found;
+                    bool seam = false;            // does the neighbourhood cross the theta seam (then mirrored rows change too)
+                    for (int idx = lane; idx < side * side; idx += 32) {
+                        int jj = j + idx / side - R, kk = k + idx % side - R;
+                        if (kk < 0 || kk >= p.n_rho) continue;
+                        if (jj < 0 || jj >= p.n_theta) {
+                            if (!p.theta_wrap) continue;
+                            while (jj < 0) { jj += p.n_theta; kk = p.n_rho - 1 - kk; }
+                            while (jj >= p.n_theta) { jj -= p.n_theta; kk = p.n_rho - 1 - kk; }
+                        }
+                        const int jl = jj - col0;
+                        const unsigned woff = (unsigned)kk * pitch + 4u * cell_word_off<ACC16>(jl);
+                        if (!HB_CHK(jl >= 0 && jl < ncols && woff + 4 <= limit, HB_H4)) continue;
+                        const unsigned mask = ACC16 ? (0xFFFFu << (16 * ((jl >> 5) & 1))) : 0xFFFFFFFFu;
+                        atomicAnd((unsigned*)(acc + woff), ~mask);     // two columns share a u16 word: clear one half atomically
+                    }
+                    if (p.theta_wrap && (j - R < 0 || j + R >= p.n_theta)) seam = true;
+                    __syncwarp();
+                    for (int kk = k - R; kk <= k + R; ++kk) {
+                        if (kk < 0 || kk >= p.n_rho) continue;
+                        const ull b = row_best(kk);
+                        if (lane == 0) rowkey[kk] = b;
+                        if (seam) {
+                            const ull bm = row_best(p.n_rho - 1 - kk);
+                            if (lane == 0) rowkey[p.n_rho - 1 - kk] = bm;
+                        }
+                    }
+                    __syncwarp();
+                    best = global_best();
+                }
+                if (lane == 0) misc[43] = n_found;
+            }
+            __syncthreads();
+            const int n_found = misc[43];
+            if (tid == 0) p.counts[2 * e] = n_found;
+            n_stored = min(n_found, p.max_peaks);
+        } else {
         // ---- H4: threshold + 3x3 local maximum -> peak bitmap (reading Q8)
         {
             // 3x3 test of one cell (reading Q8).  Branch-free: every neighbour is loaded from a clamped (always
@@ -410,8 +521,10 @@ __global__ void __launch_bounds__(1024, 1) hough_event_kernel(const __grid_const
                 unsigned nb[3][3];
 #pragma unroll
                 for (int dj = -1; dj <= 1; ++dj) {
-                    const int jj = j + dj;
-                    const bool vj = jj >= 0 && jj < p.n_theta;
+                    int jj = j + dj;
+                    bool vj = jj >= 0 && jj < p.n_theta;
+                    bool mir = false;       // EXT, theta wrap (reading Q19): column -1 is column n_theta-1 read upside down
+                    if (EXT && p.theta_wrap && !vj) { jj += jj < 0 ? p.n_theta : -p.n_theta; mir = true; vj = true; }
                     const int jc = min(max(jj, 0), p.n_theta - 1);
                     const unsigned char* base = acc;
                     int jcl = jc;
@@ -422,11 +535,13 @@ __global__ void __launch_bounds__(1024, 1) hough_event_kernel(const __grid_const
                     }
                     const unsigned char* colp = base + 4u * cell_word_off<ACC16>(jcl);
                     const int sh = ACC16 ? 16 * ((jcl >> 5) & 1) : 0;
-                    const bool in = HB_CHK(jcl >= 0 && jcl < p.cols_per_cta && km >= 0 && kp1 < p.n_rho &&
-                                           (unsigned)kp1 * pitch + 4u * cell_word_off<ACC16>(jcl) + 4 <= limit, HB_H4);
-                    const unsigned w0 = in ? *(const unsigned*)(colp + (size_t)km * p.pitch_b) : 0u;
-                    const unsigned w1 = in ? *(const unsigned*)(colp + (size_t)k * p.pitch_b) : 0u;
-                    const unsigned w2 = in ? *(const unsigned*)(colp + (size_t)kp1 * p.pitch_b) : 0u;
+                    const int r0 = (EXT && mir) ? p.n_rho - 1 - km : km, r1 = (EXT && mir) ? p.n_rho - 1 - k : k,
+                              r2 = (EXT && mir) ? p.n_rho - 1 - kp1 : kp1;
+                    const bool in = HB_CHK(jcl >= 0 && jcl < p.cols_per_cta && min(r0, r2) >= 0 && max(r0, r2) < p.n_rho &&
+                                           (unsigned)max(r0, r2) * pitch + 4u * cell_word_off<ACC16>(jcl) + 4 <= limit, HB_H4);
+                    const unsigned w0 = in ? *(const unsigned*)(colp + (size_t)r0 * p.pitch_b) : 0u;
+                    const unsigned w1 = in ? *(const unsigned*)(colp + (size_t)r1 * p.pitch_b) : 0u;
+                    const unsigned w2 = in ? *(const unsigned*)(colp + (size_t)r2 * p.pitch_b) : 0u;
                     const unsigned msk = ACC16 ? 0xFFFFu : 0xFFFFFFFFu;
                     nb[dj + 1][0] = (vj && vkm) ? ((w0 >> sh) & msk) : 0u;
                     nb[dj + 1][1] = vj ? ((w1 >> sh) & msk) : 0u;
@@ -550,13 +665,14 @@ __global__ void __launch_bounds__(1024, 1) hough_event_kernel(const __grid_const
             }
         }
         if (rank == 0 && tid == 0) p.counts[2 * e] = n_peaks;
-        const int n_stored = min(n_peaks, p.max_peaks);
+        n_stored = min(n_peaks, p.max_peaks);
         if (CL) {
             __threadfence();
             cg::this_cluster().sync();   // (C) stored peaks visible cluster-wide; accumulator region is dead
         } else {
             __syncthreads();
         }
+        }   // peak mode
 
         // ---- H6 set-up.  Marked columns = theta columns inside some stored peak's window; they get consecutive
         // indices q.  W8[q/8][k] is a byte whose bit (q%8) says "bin k of marked column q lies in a stored peak's
@@ -565,6 +681,21 @@ __global__ void __launch_bounds__(1024, 1) hough_event_kernel(const __grid_const
         float* mcf = (float*)(acc + p.mcf_off);
         float* msf = (float*)(acc + p.msf_off);
         int* colq = (int*)(acc + p.colq_off);
+        int n_marked = 0, n_g8 = 0, n_circ = 0;
+        double* circ = (double*)(acc + p.w8_off);   // EXT, distance filter: (x_c, y_c, r_c) of the first circ_cap stored peaks
+        if (EXT && p.keep_mode == 1) {
+            // ---- N4b set-up (reading Q20): the stored peaks' candidate circles, Eq. (2)
+            n_circ = min(n_stored, p.circ_cap);
+            for (int q = tid; q < n_circ; q += nthreads) {
+                const hough_peak pk = p.peaks[(size_t)e * p.max_peaks + q];
+                double xc, yc, rc;
+                circle_of(p.cos_t[pk.theta_bin], p.sin_t[pk.theta_bin], (int)pk.rho_bin, p.inv, p.rho_max, p.scale, xc, yc, rc);
+                if (HB_CHK(p.w8_off + 24 * (q + 1) <= (CL ? p.stash_off : p.region_bytes), HB_H6_SETUP)) {
+                    circ[3 * q] = xc; circ[3 * q + 1] = yc; circ[3 * q + 2] = rc;
+                }
+            }
+            __syncthreads();
+        } else {
         {
             long long cols_ub = (long long)n_stored * (2LL * p.window + 1);
             if (cols_ub > p.n_theta) cols_ub = p.n_theta;
@@ -580,6 +711,14 @@ __global__ void __launch_bounds__(1024, 1) hough_event_kernel(const __grid_const
         __syncthreads();
         for (int q = tid; q < n_stored; q += nthreads) {
             const hough_peak pk = p.peaks[(size_t)e * p.max_peaks + q];
+            if (EXT && p.theta_wrap) {     // reading Q19: window columns beyond a border fold onto the other end
+                for (int dj = -p.window; dj <= p.window; ++dj) {
+                    int j = ((int)pk.theta_bin + dj) % p.n_theta;
+                    if (j < 0) j += p.n_theta;
+                    if (HB_CHK(j >= 0 && j < p.n_theta, HB_H6_SETUP)) colq[j] = 1;
+                }
+                continue;
+            }
             const int jlo = max(0, (int)pk.theta_bin - p.window), jhi = min(p.n_theta - 1, (int)pk.theta_bin + p.window);
             for (int j = jlo; j <= jhi; ++j)
                 if (HB_CHK(j >= 0 && j < p.n_theta, HB_H6_SETUP)) colq[j] = 1;
@@ -603,19 +742,18 @@ __global__ void __launch_bounds__(1024, 1) hough_event_kernel(const __grid_const
             }
         }
         __syncthreads();
-        const int n_marked = misc[41];
-        const int n_g8 = (n_marked + 7) >> 3;
+        n_marked = misc[41];
+        n_g8 = (n_marked + 7) >> 3;
         if (tid < 8 * n_g8 - n_marked && HB_CHK(n_marked + tid < p.n_theta + 8, HB_H6_SETUP)) {   // pad the last group with columns whose bits are never set
             mcf[n_marked + tid] = 0.0f;
             msf[n_marked + tid] = 0.0f;
         }
         for (int q = tid; q < n_stored; q += nthreads) {
             const hough_peak pk = p.peaks[(size_t)e * p.max_peaks + q];
-            const int jlo = max(0, (int)pk.theta_bin - p.window), jhi = min(p.n_theta - 1, (int)pk.theta_bin + p.window);
-            const int klo = max(0, (int)pk.rho_bin - p.window), khi = min(p.n_rho - 1, (int)pk.rho_bin + p.window);
-            for (int j = jlo; j <= jhi; ++j) {
+            // sets bit (cq % 8) of bytes klo..khi of marked column j's row
+            auto fill = [&](int j, int klo, int khi) {
                 const int cq = colq[j];
-                if (!HB_CHK(cq >= 0 && cq < n_marked && ((cq >> 3) + 1) * p.w8_pitch <= p.mcf_off - p.w8_off && (khi | 3) < p.w8_pitch, HB_H6_SETUP)) continue;
+                if (!HB_CHK(cq >= 0 && cq < n_marked && ((cq >> 3) + 1) * p.w8_pitch <= p.mcf_off - p.w8_off && (khi | 3) < p.w8_pitch, HB_H6_SETUP)) return;
                 const unsigned bit4 = (1u << (cq & 7)) * 0x01010101u;
                 const unsigned row_s = (unsigned)__cvta_generic_to_shared(W8 + (cq >> 3) * p.w8_pitch);
                 for (int wd = klo >> 2; wd <= khi >> 2; ++wd) {
@@ -623,13 +761,46 @@ __global__ void __launch_bounds__(1024, 1) hough_event_kernel(const __grid_const
                     const unsigned bytes = (0xFFFFFFFFu >> (8 * (3 - b))) & (0xFFFFFFFFu << (8 * a));
                     red_shared_or(row_s + 4u * wd, bit4 & bytes);
                 }
+            };
+            if (EXT && p.theta_wrap) {     // a folded column is compared with the MIRRORED peak bin (once per fold)
+                for (int dj = -p.window; dj <= p.window; ++dj) {
+                    int j = (int)pk.theta_bin + dj, kref = (int)pk.rho_bin;
+                    while (j < 0) { j += p.n_theta; kref = p.n_rho - 1 - kref; }
+                    while (j >= p.n_theta) { j -= p.n_theta; kref = p.n_rho - 1 - kref; }
+                    fill(j, max(0, kref - p.window), min(p.n_rho - 1, kref + p.window));
+                }
+                continue;
             }
+            const int jlo = max(0, (int)pk.theta_bin - p.window), jhi = min(p.n_theta - 1, (int)pk.theta_bin + p.window);
+            const int klo = max(0, (int)pk.rho_bin - p.window), khi = min(p.n_rho - 1, (int)pk.rho_bin + p.window);
+            for (int j = jlo; j <= jhi; ++j) fill(j, klo, khi);
         }
         __syncthreads();
+        }   // keep mode
 
         // keep test of one hit: OR over the marked columns q of bit q of W8[.][bin(i, column q)]  (== S5)
         const unsigned n_rho_u = (unsigned)p.n_rho;
-        auto keep_test = [&](float2 uv, bool valid) -> bool {
+        auto keep_test = [&](float2 uv, float2 h, bool valid) -> bool {
+            if (EXT && p.keep_mode == 1) {
+                // N4b: keep iff | ||hit - centre|| - r_c | < tol for some stored peak (fp64, one rounding per operation)
+                bool kp = false;
+                if (valid) {
+                    const double x = (double)h.x, y = (double)h.y;
+                    for (int q = 0; q < n_stored && !kp; ++q) {
+                        double xc, yc, rc;
+                        if (q < n_circ) {
+                            xc = circ[3 * q]; yc = circ[3 * q + 1]; rc = circ[3 * q + 2];
+                        } else {                 // more stored peaks than staged circles: straight from the peak list
+                            const hough_peak pk = p.peaks[(size_t)e * p.max_peaks + q];
+                            circle_of(p.cos_t[pk.theta_bin], p.sin_t[pk.theta_bin], (int)pk.rho_bin, p.inv, p.rho_max, p.scale, xc, yc, rc);
+                        }
+                        const double dx = __dsub_rn(x, xc), dy = __dsub_rn(y, yc);
+                        const double d = sqrt(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)));
+                        if (fabs(__dsub_rn(d, rc)) < p.keep_tol) kp = true;
+                    }
+                }
+                return kp;
+            }
             unsigned hitbits = 0;
             for (int g8 = 0; g8 < n_g8; ++g8) {
                 if (!HB_CHK(8 * g8 + 8 <= p.n_theta + 8 && (g8 + 1) * p.w8_pitch <= p.mcf_off - p.w8_off && p.n_rho < p.w8_pitch, HB_KEEP)) break;
@@ -656,7 +827,9 @@ __global__ void __launch_bounds__(1024, 1) hough_event_kernel(const __grid_const
                 const bool valid = i < n;
                 float2 uv = make_float2(0.0f, 0.0f);
                 if (valid) uv = single ? hb[i] : conformal(__ldg(&p.xy[beg + i]), p.scale);
-                const bool kp = keep_test(uv, valid);
+                float2 hxy = make_float2(0.0f, 0.0f);
+                if (EXT && p.keep_mode == 1 && valid) hxy = __ldg(&p.xy[beg + i]);
+                const bool kp = keep_test(uv, hxy, valid);
                 int blk_total;
                 const int ppos = block_exscan(kp ? 1 : 0, misc, blk_total);
                 if (valid) {
@@ -685,7 +858,9 @@ __global__ void __launch_bounds__(1024, 1) hough_event_kernel(const __grid_const
                     const bool valid = i < n;
                     float2 uv = make_float2(0.0f, 0.0f);
                     if (valid) uv = single ? hb[i] : conformal(__ldg(&p.xy[beg + i]), p.scale);
-                    const bool kp = keep_test(uv, valid);
+                    float2 hxy = make_float2(0.0f, 0.0f);
+                    if (EXT && p.keep_mode == 1 && valid) hxy = __ldg(&p.xy[beg + i]);
+                    const bool kp = keep_test(uv, hxy, valid);
                     const unsigned bal = __ballot_sync(0xffffffffu, kp);
                     if (lane == 0 && HB_CHK(bl < HOUGH_SEL_ROUND_BLOCKS, HB_H7)) stash[bl * nwarps + warp] = bal;
                     if (valid) p.keep[beg + i] = kp ? 1 : 0;
@@ -736,6 +911,76 @@ __global__ void __launch_bounds__(1024, 1) hough_event_kernel(const __grid_const
             if (m && tid == 0) { p.counts[2 * e] = HOUGH_DBG_SENTINEL; p.counts[2 * e + 1] = m; }
         }
 #endif
+    }
+}
+
+
+// ---------------------------------------------------------------- N1: candidate circles and track parameters
+// SURVEY.md 8(f) NEXT-1; Eq. (2), pT and phi0 PAPER.md:150-158; readings Q14-Q17.
+// One CTA per event, one warp per stored peak: the lanes stride over the event's hits, count the hits ASSOCIATED with
+// the peak (own bin at the peak's column within the keep window) and on which side of the centre direction they lie
+// (fp32 cross product c_j y - s_j x, one rounding per operation); lane 0 then writes the circle in fp64.
+struct CParams {
+    const float2* xy;
+    const int* off;
+    int n_events;
+    const hough_peak* peaks;
+    const int* counts;
+    hough_circle* out;
+    const float* cos_t;
+    const float* sin_t;
+    int n_theta, n_rho, window, max_peaks;
+    float rho_max, inv, scale;
+    double b_field;
+};
+
+__global__ void __launch_bounds__(256) hough_circles_kernel(const __grid_constant__ CParams p) {
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarps = blockDim.x >> 5;
+    const double pi = 3.14159265358979323846;
+    for (int e = blockIdx.x; e < p.n_events; e += gridDim.x) {
+        const int beg = p.off[e], n = p.off[e + 1] - beg;
+        const int n_peaks = p.counts[2 * e];
+        const int n_stored = n_peaks < p.max_peaks ? n_peaks : p.max_peaks;   // a refused event (-1) stores nothing
+        for (int q = warp; q < n_stored; q += nwarps) {
+            const hough_peak pk = p.peaks[(size_t)e * p.max_peaks + q];
+            const int j = pk.theta_bin, k = pk.rho_bin;
+            const float cj = p.cos_t[j], sj = p.sin_t[j];
+            const double rc = rho_centre(k, p.inv, p.rho_max);
+            int n_pos = 0, n_neg = 0, n_assoc = 0;
+            for (int i = lane; i < n; i += 32) {
+                const float2 h = __ldg(&p.xy[beg + i]);
+                const float2 uv = conformal(h, p.scale);
+                const int kb = bin_exact(uv.x, uv.y, cj, sj, p.rho_max, p.inv, p.n_rho);
+                if (kb < 0) continue;
+                const int dk = kb > k ? kb - k : k - kb;
+                if (dk > p.window) continue;
+                ++n_assoc;
+                float z = __fsub_rn(__fmul_rn(cj, h.y), __fmul_rn(sj, h.x));
+                if (rc < 0.0) z = -z;
+                if (z > 0.0f) ++n_pos;
+                else if (z < 0.0f) ++n_neg;
+            }
+#pragma unroll
+            for (int d = 16; d >= 1; d >>= 1) {
+                n_pos += __shfl_xor_sync(0xffffffffu, n_pos, d);
+                n_neg += __shfl_xor_sync(0xffffffffu, n_neg, d);
+                n_assoc += __shfl_xor_sync(0xffffffffu, n_assoc, d);
+            }
+            if (lane == 0) {
+                hough_circle c;
+                circle_of(cj, sj, k, p.inv, p.rho_max, p.scale, c.x_c, c.y_c, c.r_c);
+                c.pt = __dmul_rn(__dmul_rn(0.0003, p.b_field), c.r_c);
+                c.charge = n_neg > n_pos ? 1 : (n_pos > n_neg ? -1 : 0);
+                c.n_hits = n_assoc;
+                double phi_c = __ddiv_rn(__dmul_rn((double)j, pi), (double)p.n_theta);
+                if (rc < 0.0) phi_c = __dadd_rn(phi_c, pi);
+                double phi0 = __dsub_rn(phi_c, __dmul_rn((double)c.charge, pi / 2.0));
+                if (phi0 < 0.0) phi0 = __dadd_rn(phi0, 2.0 * pi);
+                if (phi0 >= 2.0 * pi) phi0 = __dsub_rn(phi0, 2.0 * pi);
+                c.phi0 = phi0;
+                p.out[(size_t)e * p.max_peaks + q] = c;
+            }
+        }
     }
 }
 

@@ -12,6 +12,9 @@ import tempfile
 
 import numpy as np
 
+# the layout of hough_circle (include/hough.h)
+CIRCLE_DTYPE = np.dtype([("x_c", "<f8"), ("y_c", "<f8"), ("r_c", "<f8"), ("pt", "<f8"), ("phi0", "<f8"), ("charge", "<i4"), ("n_hits", "<i4")])
+
 HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(os.path.dirname(HERE))
 SOURCES = [os.path.join(HERE, "emu_main.cpp"), os.path.join(HERE, "simt_shim.h"),
@@ -35,7 +38,8 @@ def build(debug_bounds: bool = False, force: bool = False) -> str:
 
 
 def run(xy, off, n_theta, n_rho, rho_max, threshold, window, table, max_peaks=64, acc_dtype="u16", accum=True,
-        conformal_scale=1, cluster_size=0, ctas_per_sm=0, vote_path=0, grid_clusters=0, debug_bounds=False, timeout=600):
+        conformal_scale=1, cluster_size=0, ctas_per_sm=0, vote_path=0, grid_clusters=0, debug_bounds=False, timeout=900,
+        peak_mode=0, rel_permille=500, nms_radius=1, theta_wrap=False, keep_mode=0, keep_tol=0.0, b_field=1.0, circles=False):
     """Same arguments and result keys as tests/test_parity_gpu.py::gpu_run."""
     import paper_2607_04067_b200 as hb
     xy = np.ascontiguousarray(xy, dtype=np.float32).reshape(-1, 2)
@@ -52,13 +56,15 @@ def run(xy, off, n_theta, n_rho, rho_max, threshold, window, table, max_peaks=64
     inv = np.float32(float(n_rho) / (2.0 * rho_max32))
     head = [n_theta, n_rho, threshold, window, max_peaks, int(plan["acc_bits"] == 16), int(plan["cluster_size"] > 1),
             plan["cols_per_lane"], plan["cluster_size"], plan["threads"], plan["smem_bytes"], int(vote_path == 1),
-            n_events, n_total, 1, int(accum), grid_clusters, 0, 0, 0]
+            n_events, n_total, 1, int(accum), grid_clusters, peak_mode, rel_permille, nms_radius, int(bool(theta_wrap)), keep_mode,
+            int(circles), 0]
     with tempfile.TemporaryDirectory() as d:
         fin, fout = os.path.join(d, "in.bin"), os.path.join(d, "out.bin")
         with open(fin, "wb") as f:
-            f.write(struct.pack("<20i", *head))
-            f.write(struct.pack("<26i", *fields))
+            f.write(struct.pack("<24i", *head))
+            f.write(struct.pack("<27i", *fields))
             f.write(struct.pack("<5f", rho_max32, float(inv), float(conformal_scale), tame, ftz_min))
+            f.write(struct.pack("<2d", float(keep_tol), float(b_field)))
             f.write(c.tobytes()); f.write(s.tobytes()); f.write(off.tobytes()); f.write(xy.tobytes())
         r = subprocess.run([build(debug_bounds), fin, fout], capture_output=True, text=True, timeout=timeout)
         if r.returncode != 0:
@@ -77,6 +83,8 @@ def run(xy, off, n_theta, n_rho, rho_max, threshold, window, table, max_peaks=64
            "kept_idx": take(n_total, np.int32)}
     if accum:
         res["accum"] = take(n_events * n_theta * n_rho, np.int32).reshape(n_events, n_theta, n_rho)
+    if circles:
+        res["circles"] = take(n_events * max_peaks, CIRCLE_DTYPE).reshape(n_events, max_peaks)
     res["peaks3"] = hb.unpack_peaks(res["peaks"])
     res["info"] = {"CLUSTER_SIZE": plan["cluster_size"], "THREADS": plan["threads"], "SMEM_BYTES": plan["smem_bytes"],
                    "ACC_BITS": plan["acc_bits"], "CHUNK_HITS": plan["chunk_hits"]}

@@ -15,19 +15,26 @@ namespace {
 hough::KParams kp;
 int g_acc16, g_cl, g_cpl;
 
-template <bool ACC16, bool CL>
+int g_ext;
+hough::CParams cpar;
+
+template <bool ACC16, bool CL, bool EXT>
 void call_cpl() {
     switch (g_cpl) {
-        case 6: hough::hough_event_kernel<ACC16, CL, 6>(kp); break;
-        case 4: hough::hough_event_kernel<ACC16, CL, 4>(kp); break;
-        default: hough::hough_event_kernel<ACC16, CL, 2>(kp); break;
+        case 6: hough::hough_event_kernel<ACC16, CL, 6, EXT>(kp); break;
+        case 4: hough::hough_event_kernel<ACC16, CL, 4, EXT>(kp); break;
+        default: hough::hough_event_kernel<ACC16, CL, 2, EXT>(kp); break;
     }
 }
 
-void entry() {
-    if (g_acc16) { if (g_cl) call_cpl<true, true>(); else call_cpl<true, false>(); }
-    else { if (g_cl) call_cpl<false, true>(); else call_cpl<false, false>(); }
+template <bool EXT>
+void entry_t() {
+    if (g_acc16) { if (g_cl) call_cpl<true, true, EXT>(); else call_cpl<true, false, EXT>(); }
+    else { if (g_cl) call_cpl<false, true, EXT>(); else call_cpl<false, false, EXT>(); }
 }
+
+void entry() { if (g_ext) entry_t<true>(); else entry_t<false>(); }   // the same choice hough_api.cu's pick_kernel makes
+void entry_circles() { hough::hough_circles_kernel(cpar); }
 
 template <class T> void rd(FILE* f, T* p, size_t n) {
     if (n && fread(p, sizeof(T), n, f) != n) emu::die("short input file");
@@ -39,15 +46,18 @@ int main(int argc, char** argv) {
     if (argc != 3) emu::die("usage: hough_emu in.bin out.bin");
     FILE* f = fopen(argv[1], "rb");
     if (!f) emu::die("cannot open the input file");
-    // header: 20 ints, 26 plan fields (int32), 5 floats
-    int h[20];
-    int plan[26];
+    // header: 24 ints, 27 plan fields (int32), 5 floats, 2 doubles
+    int h[24];
+    int plan[27];
     float fl[5];
-    rd(f, h, 20); rd(f, plan, 26); rd(f, fl, 5);
+    double dbl[2];
+    rd(f, h, 24); rd(f, plan, 27); rd(f, fl, 5); rd(f, dbl, 2);
     const int n_theta = h[0], n_rho = h[1], threshold = h[2], window = h[3], max_peaks = h[4];
     g_acc16 = h[5]; g_cl = h[6]; g_cpl = h[7];
     const int csize = h[8], threads = h[9], smem_bytes = h[10], force_slow = h[11], n_events = h[12], n_total = h[13];
     const int want_kept = h[14], want_accum = h[15], grid_clusters = h[16];
+    const int peak_mode = h[17], rel_permille = h[18], nms_radius = h[19], theta_wrap = h[20], keep_mode = h[21], want_circles = h[22];
+    g_ext = peak_mode != 0 || theta_wrap != 0 || keep_mode != 0;
     std::vector<float> cos_t(n_theta), sin_t(n_theta);
     rd(f, cos_t.data(), n_theta); rd(f, sin_t.data(), n_theta);
     emu::Guarded b_off, b_xy, b_keep, b_peaks, b_counts, b_kxy, b_kidx, b_acc;
@@ -87,7 +97,10 @@ int main(int argc, char** argv) {
     kp.chunk = plan[10]; kp.region_bytes = plan[11]; kp.pbm_off = plan[12]; kp.pbm_bytes = plan[13]; kp.hb_off = plan[14];
     kp.misc_off = plan[15]; kp.w8_off = plan[16]; kp.w8_pitch = plan[17]; kp.mcf_off = plan[18]; kp.msf_off = plan[19];
     kp.colq_off = plan[20]; kp.stash_off = plan[21]; kp.cnt_off = plan[22]; kp.gcnt_off = plan[23];
-    kp.rcp_groups = (unsigned)plan[24]; kp.rcp_2s = (unsigned)plan[25];
+    kp.rcp_groups = (unsigned)plan[24]; kp.rcp_2s = (unsigned)plan[25]; kp.circ_cap = plan[26];
+    kp.peak_mode = peak_mode; kp.rel_permille = rel_permille; kp.nms_radius = nms_radius; kp.theta_wrap = theta_wrap;
+    kp.keep_mode = keep_mode; kp.keep_tol = dbl[0];
+    if (peak_mode == 1 && csize > 1) emu::die("peak mode 1 needs one CTA per event (hough_run refuses this too)");
     kp.vpr = kp.pitch_b / 16;
     if (plan[0] != csize || plan[1] != threads || plan[2] != smem_bytes || plan[4] != g_cpl || (plan[3] == 16) != (g_acc16 != 0))
         emu::die("header and plan disagree");
@@ -95,6 +108,21 @@ int main(int argc, char** argv) {
     // hough_run launches one cluster per event; a smaller grid also exercises the kernel's event loop
     const int n_clusters = grid_clusters > 0 ? (grid_clusters < n_events ? grid_clusters : n_events) : n_events;
     for (int c = 0; c < n_clusters; ++c) emu::run_cluster(c, n_clusters, csize, threads, (size_t)smem_bytes, entry);
+
+    // N1: hough_circles on the peaks just written (grid = one 256-thread CTA per event, as hough_api.cu launches it)
+    emu::Guarded b_circ;
+    const size_t circ_bytes = sizeof(hough_circle) * (size_t)n_events * max_peaks;
+    b_circ.alloc(circ_bytes + sizeof(hough_circle));
+    memset(b_circ.ptr, 0xFF, b_circ.bytes);
+    if (want_circles && max_peaks > 0) {
+        cpar = hough::CParams();
+        cpar.xy = kp.xy; cpar.off = kp.off; cpar.n_events = n_events; cpar.peaks = kp.peaks; cpar.counts = kp.counts;
+        cpar.out = (hough_circle*)(b_circ.ptr + sizeof(hough_circle)); cpar.cos_t = kp.cos_t; cpar.sin_t = kp.sin_t;
+        cpar.n_theta = n_theta; cpar.n_rho = n_rho; cpar.window = window; cpar.max_peaks = max_peaks;
+        cpar.rho_max = kp.rho_max; cpar.inv = kp.inv; cpar.scale = kp.scale; cpar.b_field = dbl[1];
+        const int cgrid = grid_clusters > 0 ? (grid_clusters < n_events ? grid_clusters : n_events) : n_events;
+        for (int c = 0; c < cgrid; ++c) emu::run_cluster(c, cgrid, 1, 256, 16, entry_circles);
+    }
 
     FILE* o = fopen(argv[2], "wb");
     if (!o) emu::die("cannot open the output file");
@@ -104,6 +132,7 @@ int main(int argc, char** argv) {
     fwrite(b_kxy.ptr + 8, 4, 2 * (size_t)n_total, o);
     fwrite(b_kidx.ptr + 4, 4, (size_t)n_total, o);
     if (want_accum) fwrite(b_acc.ptr + 4, 1, accum_bytes, o);
+    if (want_circles) fwrite(b_circ.ptr + sizeof(hough_circle), 1, circ_bytes, o);
     fclose(o);
     return 0;
 }

@@ -178,7 +178,7 @@ inline void run_cluster(int cluster, int n_clusters, int csize, int threads, siz
         c.warps.assign((size_t)threads / 32, Warp());
         for (int t = 0; t < threads; ++t) {
             Fiber& f = fibers[(size_t)r * threads + t];
-            f.stack.resize(48 * 1024);
+            f.stack.resize(32 * 1024);
             f.tidx.x = (unsigned)t;
             f.cta = &c;
             getcontext(&f.ctx);
@@ -237,9 +237,20 @@ inline unsigned __ballot_sync(unsigned m, int p) {
     return r;
 }
 inline int __all_sync(unsigned m, int p) { return __ballot_sync(m, p) == 0xffffffffu; }
+inline int __shfl_xor_sync(unsigned m, int v, int d) {
+    need_full_mask(m);
+    const int lane = (int)(emu::cur->tidx.x & 31);
+    return (int)emu::warp_exchange((unsigned)v)[(lane ^ d) & 31];
+}
+inline unsigned long long __shfl_xor_sync(unsigned m, unsigned long long v, int d) {
+    const unsigned lo = (unsigned)__shfl_xor_sync(m, (int)(unsigned)v, d), hi = (unsigned)__shfl_xor_sync(m, (int)(unsigned)(v >> 32), d);
+    return (unsigned long long)lo | ((unsigned long long)hi << 32);
+}
+inline void __syncwarp() { emu::warp_exchange(0u); }
 
 inline unsigned atomicAdd(unsigned* p, unsigned v) { unsigned o = *p; *p = o + v; return o; }
 inline int atomicAdd(int* p, int v) { int o = *p; *p = o + v; return o; }
+inline unsigned atomicAnd(unsigned* p, unsigned v) { unsigned o = *p; *p = o & v; return o; }
 template <class T> inline T __ldg(const T* p) { return *p; }
 inline size_t __cvta_generic_to_shared(const void* p) {
     const ptrdiff_t off = (const unsigned char*)p - emu::cur->cta->smem.ptr;
@@ -253,6 +264,11 @@ inline float __uint_as_float(unsigned u) { float f; memcpy(&f, &u, 4); return f;
 inline float __fmul_rn(float a, float b) { volatile float r = a * b; return r; }
 inline float __fadd_rn(float a, float b) { volatile float r = a + b; return r; }
 inline float __fdiv_rn(float a, float b) { volatile float r = a / b; return r; }
+inline float __fsub_rn(float a, float b) { volatile float r = a - b; return r; }
+inline double __dadd_rn(double a, double b) { volatile double r = a + b; return r; }
+inline double __dsub_rn(double a, double b) { volatile double r = a - b; return r; }
+inline double __dmul_rn(double a, double b) { volatile double r = a * b; return r; }
+inline double __ddiv_rn(double a, double b) { volatile double r = a / b; return r; }
 inline float __fadd_rd(float a, float b) {        // round toward minus infinity: exact in double, then step down if needed
     const double s = (double)a + (double)b;
     float r = (float)s;

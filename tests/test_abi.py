@@ -14,7 +14,7 @@ ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 def declared_functions(header):
     src = open(os.path.join(ROOT, "include", header)).read()
     src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
-    return sorted(set(re.findall(r"\b(hough_[a-z_]+)\s*\(", src)))
+    return sorted(set(re.findall(r"\b(hough_[a-z_0-9]+)\s*\(", src)))
 
 
 def test_libraries_export_every_symbol_the_headers_declare():

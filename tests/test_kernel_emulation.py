@@ -75,3 +75,78 @@ def test_truncation_and_window_under_the_emulator():
     xy, off, _ = si.generate(w, 1)
     emu_both(w, xy, off, max_peaks=3, window=2, debug_bounds=True)
     emu_both(w, xy, off, max_peaks=0)
+
+
+# ---------------------------------------------------------------- the NEXT rows under the emulator (against oracle.run_ex)
+def emu_ex(w, xy, off, accum=True, circles=False, **kw):
+    table = si.trig_table(w.n_theta)
+    base = dict(max_peaks=w.max_peaks, acc_dtype=w.acc_dtype, threshold=w.threshold, window=w.window, conformal_scale=1)
+    base.update({k: kw.pop(k) for k in list(kw) if k in base})
+    opts = {k: kw.pop(k) for k in list(kw) if k in ("peak_mode", "rel_permille", "nms_radius", "theta_wrap", "keep_mode", "keep_tol", "b_field")}
+    rho_max = kw.pop("rho_max", w.rho_max)
+    g = simt_emu.run(xy, off, w.n_theta, w.n_rho, rho_max, base["threshold"], base["window"], table, max_peaks=base["max_peaks"],
+                     acc_dtype=base["acc_dtype"], accum=accum, conformal_scale=base["conformal_scale"], circles=circles, **opts, **kw)
+    o, oc = oracle.run_ex(xy, off, w.n_theta, w.n_rho, rho_max, base["threshold"], base["window"], table[0], table[1],
+                          max_peaks=base["max_peaks"], conformal_scale=base["conformal_scale"], acc_u16=(base["acc_dtype"] != "u32"),
+                          want_accum=accum, n_threads=4, want_circles=circles, **opts)
+    assert not np.any(g["counts"][:, 0] == -2), "debug-bounds sentinel: phases %s" % g["counts"][g["counts"][:, 0] == -2, 1]
+    compare(g, o, off, base["max_peaks"], accum=accum, tag=w.name)
+    if circles:
+        for e in range(len(off) - 1):
+            ns = min(int(o.counts[e, 0]), base["max_peaks"])
+            assert g["circles"][e, :ns].tobytes() == oc[e, :ns].tobytes(), "circles of event %d" % e     # bit for bit, fp64 included
+            assert np.all(np.frombuffer(g["circles"][e, ns:].tobytes(), dtype=np.uint8) == 0xFF)           # the rest is untouched
+    return g, o
+
+
+def test_n1_circles_under_the_emulator():
+    w = si.config(0)
+    xy, off, _ = si.generate(w, 3)
+    emu_ex(w, xy, off, circles=True, debug_bounds=True, b_field=1.0)
+    emu_ex(w, xy, off, circles=True, conformal_scale=2, rho_max=float(np.float32(2) * np.float32(w.rho_max)), b_field=0.8)
+    w1 = si.config(0, 1)
+    w1 = type(w1)(**{**w1.__dict__, "n_theta": 4, "n_rho": 8, "rho_max": 2.0, "threshold": 2, "window": 0, "max_peaks": 8})
+    xy1 = np.array([[1, 0], [0, 1], [.5, .5], [-1, 0], [0, 0], [4, 0]], dtype=np.float32)
+    g, _ = emu_ex(w1, xy1, np.array([0, 6], dtype=np.int32), circles=True)
+    assert [int(c) for c in g["circles"][0, :3]["charge"]] == [-1, -1, 1] and g["circles"][0, 2]["r_c"] == 2.0     # tests/golden/w1_next.txt
+
+
+@pytest.mark.parametrize("cfg,permille,radius,wrap", [(0, 500, 1, False), (1, 300, 2, False), (0, 0, 0, True), (3, 600, 3, True)])
+def test_n2_iterative_nms_under_the_emulator(cfg, permille, radius, wrap):
+    w = si.config(cfg)
+    xy, off, _ = si.generate(w, 2 if cfg != 3 else 1)
+    g, o = emu_ex(w, xy, off, peak_mode=1, rel_permille=permille, nms_radius=radius, theta_wrap=wrap, debug_bounds=True)
+    assert o.counts[:, 0].min() >= 1
+    emu_ex(w, xy, off, peak_mode=1, rel_permille=permille, nms_radius=radius, theta_wrap=wrap, max_peaks=2)
+
+
+@pytest.mark.parametrize("cluster,window", [(0, 1), (0, 3), (2, 2)])
+def test_n4a_theta_wrap_under_the_emulator(cluster, window):
+    w = si.config(0)
+    xy, off, _ = si.generate(w, 3)
+    # a noiseless track whose centre direction (179.8 deg) sits on the theta seam: it peaks at column 0 AND, mirrored, at 179
+    r = 200.0 + np.arange(48) * 600.0 / 47.0
+    phi = np.deg2rad(179.8) - np.arccos(r / 1200.0)
+    xy = np.concatenate([np.stack([r * np.cos(phi), r * np.sin(phi)], axis=1).astype(np.float32), xy])
+    off = off.copy()
+    off[1:] += 48
+    g, o = emu_ex(w, xy, off, theta_wrap=True, window=window, threshold=12, max_peaks=512, cluster_size=cluster, debug_bounds=True)
+    o0, _ = oracle.run_ex(xy, off, w.n_theta, w.n_rho, w.rho_max, 12, window, *si.trig_table(w.n_theta), max_peaks=512)
+    assert not np.array_equal(o.keep, o0.keep) or not np.array_equal(o.counts, o0.counts)      # the seam matters on these events
+
+
+@pytest.mark.parametrize("cluster,tol", [(0, 5.0), (2, 20.0), (0, 0.0)])
+def test_n4b_distance_filter_under_the_emulator(cluster, tol):
+    w = si.config(0)
+    xy, off, _ = si.generate(w, 3)
+    emu_ex(w, xy, off, keep_mode=1, keep_tol=tol, cluster_size=cluster, debug_bounds=True)
+
+
+def test_n3_the_papers_1000x1000_grid_under_the_emulator():
+    # rho in [-0.01, 0.01] and theta in [0, pi), 1000 bins each; 0.01/mm = 2/r at r = 200 mm, i.e. the scale
+    # of Eq. (2).  2 MB of u16 cells: a 16-CTA (non-portable) cluster, 63 theta columns per CTA
+    w = si.config(0)
+    w = type(w)(**{**w.__dict__, "n_theta": 1000, "n_rho": 1000, "rho_max": 0.01, "threshold": 12, "window": 2, "max_peaks": 64})
+    xy, off, _ = si.generate(w, 1)
+    g, o = emu_ex(w, xy, off, conformal_scale=2, debug_bounds=True, accum=True)
+    assert g["info"]["CLUSTER_SIZE"] == 16 and o.counts[0, 0] >= 2

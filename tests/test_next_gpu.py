@@ -1,0 +1,181 @@
+"""-m gpu: the rows SURVEY.md 8(f) marks NEXT, through the C ABI, against oracle.run_ex, element by element and bit for
+bit (fp64 circle records included): N1 candidate circles, N2 relative threshold + iterative NMS, N3 the paper's
+1000 x 1000 grid on a 16-CTA cluster, N4a theta wrap, N4b original-space distance filter, N4c per-stream host staging."""
+import numpy as np
+import pytest
+
+import oracle
+import stcf_inputs as si
+from tests.test_parity_gpu import compare
+
+pytestmark = pytest.mark.gpu
+
+OPTS = ("peak_mode", "rel_permille", "nms_radius", "theta_wrap", "keep_mode", "keep_tol", "b_field")
+
+
+@pytest.fixture(scope="module")
+def hb():
+    import torch
+    assert torch.cuda.is_available()
+    import paper_2607_04067_b200 as m
+    m.load_library()
+    return m
+
+
+def gpu_ex(hb, w, xy, off, accum=True, circles=False, cluster_size=0, rho_max=None, **kw):
+    import torch
+    table = si.trig_table(w.n_theta)
+    base = dict(max_peaks=w.max_peaks, acc_dtype=w.acc_dtype, threshold=w.threshold, window=w.window, conformal_scale=1)
+    base.update({k: kw.pop(k) for k in list(kw) if k in base})
+    opts = {k: kw.pop(k) for k in list(kw) if k in OPTS}
+    assert not kw, kw
+    rho_max = w.rho_max if rho_max is None else rho_max
+    h = hb.Hough(w.n_theta, w.n_rho, rho_max, base["threshold"], base["window"], max_peaks=base["max_peaks"], acc_dtype=base["acc_dtype"],
+                 conformal_scale=base["conformal_scale"], cluster_size=cluster_size, trig_table=table, **opts)
+    try:
+        d_xy = torch.from_numpy(np.ascontiguousarray(xy, dtype=np.float32).reshape(-1, 2)).cuda()
+        d_off = torch.from_numpy(np.ascontiguousarray(off, dtype=np.int32)).cuda()
+        out = h.alloc_outputs(d_xy.shape[0], d_off.numel() - 1, accum=accum)
+        out["keep"].fill_(7); out["counts"].fill_(-99); out["kept_idx"].fill_(-5); out["peaks"].fill_(-1)
+        h.run(d_xy, d_off, out=out)
+        circ = h.circles(d_xy, d_off, out) if circles else None
+        torch.cuda.synchronize()
+        g = {k: v.cpu().numpy() for k, v in out.items()}
+        g["peaks3"] = hb.unpack_peaks(g["peaks"])
+        g["info"] = {"CLUSTER_SIZE": h.info(hb.HOUGH_INFO_CLUSTER_SIZE), "THREADS": h.info(hb.HOUGH_INFO_THREADS)}
+        if circ is not None:
+            g["circles"] = np.ascontiguousarray(circ.cpu().numpy()).view(hb.circle_dtype()).reshape(len(off) - 1, base["max_peaks"])
+    finally:
+        h.close()
+    o, oc = oracle.run_ex(xy, off, w.n_theta, w.n_rho, rho_max, base["threshold"], base["window"], table[0], table[1],
+                          max_peaks=base["max_peaks"], conformal_scale=base["conformal_scale"], acc_u16=(base["acc_dtype"] != "u32"),
+                          want_accum=accum, n_threads=8, want_circles=circles, **opts)
+    compare(g, o, off, base["max_peaks"], accum=accum, tag=w.name)
+    if circles:
+        for e in range(len(off) - 1):
+            ns = min(int(o.counts[e, 0]), base["max_peaks"])
+            assert g["circles"][e, :ns].tobytes() == oc[e, :ns].tobytes(), "circles of event %d" % e
+            assert not np.frombuffer(g["circles"][e, ns:].tobytes(), dtype=np.uint8).any()      # entries past the stored ones are untouched
+    return g, o, oc
+
+
+def seam_events(w, n_ev):
+    """Config-0 events with a noiseless track on the theta seam (centre direction 179.8 deg) added to the first one."""
+    xy, off, _ = si.generate(w, n_ev)
+    r = 200.0 + np.arange(48) * 600.0 / 47.0
+    phi = np.deg2rad(179.8) - np.arccos(r / 1200.0)
+    xy = np.concatenate([np.stack([r * np.cos(phi), r * np.sin(phi)], axis=1).astype(np.float32), xy])
+    off = off.copy()
+    off[1:] += 48
+    return xy, off
+
+
+# ---------------------------------------------------------------- N1
+@pytest.mark.parametrize("cfg,n_ev", [(0, 16), (1, 60), (2, 8), (3, 4)])
+def test_n1_circles_match_the_oracle_bit_for_bit(hb, cfg, n_ev):
+    w = si.config(cfg)
+    xy, off, _ = si.generate(w, n_ev)
+    g, o, oc = gpu_ex(hb, w, xy, off, circles=True, accum=False)
+    assert o.counts[:, 0].max() >= 1
+
+
+def test_n1_closed_form_worked_example_scale_2_and_b_field(hb):
+    # P1 on the GPU: r_c = 1644.31 mm, pT = 0.4933 GeV, charge and phi0 of either turning sense (tests/test_oracle_next_pins.py)
+    from tests.test_oracle_next_pins import p1_hits
+    w = si.config(0)
+    for q in (1, -1):
+        xy, R, phi_c = p1_hits(q)
+        g, o, oc = gpu_ex(hb, w, xy, np.array([0, 48], dtype=np.int32), circles=True)
+        i = g["peaks3"][0, :g["counts"][0, 0]].tolist().index([40, 70, 48])
+        c = g["circles"][0, i]
+        assert c["r_c"] == pytest.approx(1644.31, abs=0.01) and c["pt"] == pytest.approx(0.4933, abs=1e-4) and c["charge"] == q
+        assert c["phi0"] == pytest.approx((phi_c - q * np.pi / 2) % (2 * np.pi), abs=1e-9)
+    xy, off, _ = si.generate(w, 6)
+    a, _, _ = gpu_ex(hb, w, xy, off, circles=True, b_field=0.5)
+    b, _, _ = gpu_ex(hb, w, xy, off, circles=True, b_field=0.5, conformal_scale=2, rho_max=float(np.float32(2) * np.float32(w.rho_max)))
+    assert a["circles"].tobytes() == b["circles"].tobytes()
+    # W1 (tests/golden/w1_next.txt)
+    w1 = type(w)(**{**w.__dict__, "n_theta": 4, "n_rho": 8, "rho_max": 2.0, "threshold": 2, "window": 0, "max_peaks": 8})
+    xy1 = np.array([[1, 0], [0, 1], [.5, .5], [-1, 0], [0, 0], [4, 0]], dtype=np.float32)
+    g, _, _ = gpu_ex(hb, w1, xy1, np.array([0, 6], dtype=np.int32), circles=True)
+    assert [int(c) for c in g["circles"][0, :3]["charge"]] == [-1, -1, 1] and [int(c) for c in g["circles"][0, :3]["n_hits"]] == [2, 2, 3]
+    assert g["circles"][0, 2]["r_c"] == 2.0 and g["circles"][0, 2]["phi0"] == 0.0
+
+
+def test_n1_on_a_cluster_grid_and_with_empty_and_refused_events(hb):
+    w = si.config(5)
+    xy, off, _ = si.generate(w, 8)
+    off2 = np.concatenate([[0, 0], off[1:]]).astype(np.int32)         # an empty event in front
+    gpu_ex(hb, w, xy, off2, circles=True, accum=False)
+
+
+# ---------------------------------------------------------------- N2
+@pytest.mark.parametrize("cfg,n_ev,permille,radius", [(0, 16, 500, 1), (1, 64, 300, 2), (2, 6, 400, 1), (3, 4, 700, 3), (1, 20, 0, 0), (1, 20, 1000, 5)])
+def test_n2_relative_threshold_and_iterative_nms(hb, cfg, n_ev, permille, radius):
+    w = si.config(cfg)
+    xy, off, _ = si.generate(w, n_ev)
+    g, o, _ = gpu_ex(hb, w, xy, off, peak_mode=1, rel_permille=permille, nms_radius=radius)
+    assert o.counts[:, 0].max() >= 1
+    gpu_ex(hb, w, xy, off, peak_mode=1, rel_permille=permille, nms_radius=radius, max_peaks=3, accum=False)     # truncation
+
+
+def test_n2_full_batch_and_wrap_and_refusal_on_cluster_grids(hb):
+    w = si.config(1)
+    xy, off, _ = si.generate(w)                                     # the 1000-event batch
+    gpu_ex(hb, w, xy, off, peak_mode=1, rel_permille=500, nms_radius=2, accum=False)
+    w0 = si.config(0)
+    xy, off = seam_events(w0, 4)
+    gpu_ex(hb, w0, xy, off, peak_mode=1, rel_permille=300, nms_radius=2, theta_wrap=True, threshold=12)
+    w5 = si.config(5)
+    xy, off, _ = si.generate(w5, 2)
+    with pytest.raises(hb.HoughError, match="one CTA"):
+        gpu_ex(hb, w5, xy, off, peak_mode=1)
+
+
+# ---------------------------------------------------------------- N3
+def test_n3_the_papers_1000x1000_grid_on_a_16_cta_cluster(hb):
+    # rho in [-0.01, 0.01] (1/mm: 2/r at r = 200 mm, the scale of Eq. (2)), theta in [0, pi), 1000 bins each
+    w = si.config(1)
+    w = type(w)(**{**w.__dict__, "n_theta": 1000, "n_rho": 1000, "rho_max": 0.01, "threshold": 12, "window": 2, "max_peaks": 64})
+    xy, off, _ = si.generate(w, 12)
+    g, o, _ = gpu_ex(hb, w, xy, off, conformal_scale=2, circles=True)
+    assert g["info"]["CLUSTER_SIZE"] == 16 and o.counts[:, 0].min() >= 1
+    gpu_ex(hb, w, xy, off, conformal_scale=2, theta_wrap=True, keep_mode=1, keep_tol=3.0, accum=False)
+
+
+# ---------------------------------------------------------------- N4a / N4b
+@pytest.mark.parametrize("cluster,window", [(0, 1), (0, 3), (2, 2), (8, 1)])
+def test_n4a_theta_wrap(hb, cluster, window):
+    w = si.config(0)
+    xy, off = seam_events(w, 8)
+    g, o, _ = gpu_ex(hb, w, xy, off, theta_wrap=True, window=window, threshold=12, max_peaks=512, cluster_size=cluster)
+    o0, _ = oracle.run_ex(xy, off, w.n_theta, w.n_rho, w.rho_max, 12, window, *si.trig_table(w.n_theta), max_peaks=512)
+    assert not np.array_equal(o.counts, o0.counts)                    # the seam track's mirrored duplicate peak is gone
+
+
+@pytest.mark.parametrize("cfg,n_ev,cluster,tol", [(0, 16, 0, 5.0), (1, 40, 0, 2.0), (1, 12, 4, 20.0), (2, 4, 0, 1.0), (3, 3, 0, 0.5), (0, 4, 0, 0.0)])
+def test_n4b_distance_filter(hb, cfg, n_ev, cluster, tol):
+    w = si.config(cfg)
+    xy, off, _ = si.generate(w, n_ev)
+    gpu_ex(hb, w, xy, off, keep_mode=1, keep_tol=tol, cluster_size=cluster, accum=False)
+
+
+def test_n4b_more_stored_peaks_than_staged_circles(hb):
+    # a cluster stages only ~350 circles beside its compaction scratch: peaks beyond that come straight from the peak list
+    w = si.config(3)
+    xy, off, _ = si.generate(w, 2)
+    g, o, _ = gpu_ex(hb, w, xy, off, keep_mode=1, keep_tol=0.2, cluster_size=2, accum=False)
+    assert o.counts[:, 0].min() > 400
+
+
+def test_option_validation(hb):
+    h = hb.Hough(180, 128, 0.003, 10, 1)
+    for key, bad in ((hb.HOUGH_OPT_PEAK_MODE, 2), (hb.HOUGH_OPT_REL_THRESHOLD_PERMILLE, 1001), (hb.HOUGH_OPT_NMS_RADIUS, 65),
+                     (hb.HOUGH_OPT_THETA_WRAP, 2), (hb.HOUGH_OPT_KEEP_MODE, -1), (hb.HOUGH_OPT_CLUSTER_SIZE, 3)):
+        with pytest.raises(hb.HoughError):
+            hb.hough_set_option(h.ctx, key, bad)
+    with pytest.raises(hb.HoughError):
+        hb.hough_set_option_f64(h.ctx, hb.HOUGH_OPTF_KEEP_TOL, -1.0)
+    with pytest.raises(hb.HoughError):
+        hb.hough_set_option_f64(h.ctx, 99, 1.0)
+    h.close()

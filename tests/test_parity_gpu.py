@@ -363,7 +363,7 @@ def test_plain_hough_run_and_streams_and_reentrancy(hb):
     with pytest.raises(hb.HoughError):
         hb.hough_create(0, 10, 1.0, 1, 0)
     with pytest.raises(hb.HoughError):
-        hb.Hough(1000, 1000, 0.01, 10, 1)            # the paper's own grid: NEXT-3, does not fit a cluster yet
+        hb.Hough(1000, 1000, 0.01, 10, 1, acc_dtype="u32")   # 4 MB of u32 cells fit no cluster (u16 does: tests/test_next_gpu.py)
 
 
 def test_run_host_end_to_end(hb):

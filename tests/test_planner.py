@@ -17,7 +17,7 @@ MAGIC_BITS = 0x4B400000
 def check_plan(n_theta, n_rho, p):
     C = p["cluster_size"]
     cell = p["acc_bits"] // 8
-    assert C in (1, 2, 4, 8)
+    assert C in (1, 2, 4, 8, 16)
     assert p["cols_per_cta"] * C >= n_theta and p["cols_per_cta"] * (C - 1) < n_theta
     # vote mapping: every warp owns one group of 32 * CPL columns, all groups together cover the CTA's columns
     padded = 32 * p["cols_per_lane"] * p["n_groups"]
@@ -35,6 +35,8 @@ def check_plan(n_theta, n_rho, p):
     assert p["pbm_off"] == p["region_bytes"]
     assert p["bitmap_words_per_row"] == (n_rho + 31) // 32
     assert p["pbm_bytes"] >= p["cols_per_cta"] * p["bitmap_words_per_row"] * 4
+    assert p["pbm_bytes"] >= 8 * n_rho                                   # iterative NMS keeps one 8-byte key per rho row there
+    assert 0 < 24 * p["circ_cap"] <= (p["stash_off"] if C > 1 else p["region_bytes"])   # staged circles stay clear of the compaction scratch
     assert p["hb_off"] == p["pbm_off"] + p["pbm_bytes"]
     assert p["misc_off"] == p["hb_off"] + 8 * p["chunk_hits"]
     assert p["smem_bytes"] >= p["misc_off"] + 256 and p["smem_bytes"] <= SMEM_OPTIN
@@ -108,7 +110,7 @@ def reachable_bits(n_rho, rng, dense):
 def test_vote_address_map_of_the_baseline_configs_over_every_reachable_bit_pattern(cfg):
     w = si.config(cfg)
     acc = hb.HOUGH_ACC_U32 if w.acc_dtype == "u32" else hb.HOUGH_ACC_U16
-    for C in (0, 2, 4, 8):
+    for C in (0, 2, 4, 8, 16):
         try:
             p = hb.hough_plan_describe(w.n_theta, w.n_rho, acc, cluster_size=C)
         except hb.HoughError:
@@ -125,7 +127,7 @@ def test_vote_address_map_of_random_grids():
         n_rho = pr.choice([1, 2, 31, 32, 33, 128, 256, 257, 512, 1000, pr.randint(1, 2000)])
         acc = pr.choice([hb.HOUGH_ACC_U16, hb.HOUGH_ACC_U32])
         try:
-            p = hb.hough_plan_describe(n_theta, n_rho, acc, cluster_size=pr.choice([0, 0, 1, 2, 4, 8]), ctas_per_sm=pr.choice([0, 1]))
+            p = hb.hough_plan_describe(n_theta, n_rho, acc, cluster_size=pr.choice([0, 0, 1, 2, 4, 8, 16]), ctas_per_sm=pr.choice([0, 1]))
         except hb.HoughError:
             continue
         emulate_vote_addresses(p, n_rho, reachable_bits(n_rho, rng, dense=False))
@@ -181,7 +183,7 @@ def test_plans_of_the_baseline_configs(cfg):
 
 
 def test_forced_cluster_sizes_and_one_cta_per_sm():
-    for C in (1, 2, 4, 8):
+    for C in (1, 2, 4, 8, 16):
         p = hb.hough_plan_describe(360, 256, hb.HOUGH_ACC_U16, cluster_size=C)
         assert p["cluster_size"] == C
         check_plan(360, 256, p)
@@ -207,10 +209,17 @@ def test_random_grids_either_fit_with_all_invariants_or_are_refused():
     assert fitted > 100 and refused > 0
 
 
-def test_the_papers_own_grid_is_refused_for_now():
-    # 1000 x 1000 needs 2 MB of u16 cells: beyond an 8-CTA cluster
+def test_the_papers_own_grid_takes_a_16_cta_cluster():
+    # 1000 x 1000 needs 2 MB of u16 cells: beyond an 8-CTA cluster, 63 columns per CTA of a 16-CTA one
+    # (SURVEY.md 8(f) NEXT-3); 4 MB of u32 cells fit nowhere
+    p = hb.hough_plan_describe(1000, 1000, hb.HOUGH_ACC_U16)
+    assert (p["cluster_size"], p["cols_per_cta"], p["threads"]) == (16, 63, 1024)
+    check_plan(1000, 1000, p)
+    emulate_vote_addresses(p, 1000, reachable_bits(1000, None, dense=True))
     with pytest.raises(hb.HoughError):
-        hb.hough_plan_describe(1000, 1000, hb.HOUGH_ACC_U16)
+        hb.hough_plan_describe(1000, 1000, hb.HOUGH_ACC_U32)
+    # 16 is only taken when nothing smaller fits
+    assert hb.hough_plan_describe(360, 512, hb.HOUGH_ACC_U16)["cluster_size"] == 2
 
 
 def test_bad_arguments_are_rejected():

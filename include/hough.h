@@ -209,9 +209,16 @@ int hough_circles(hough_ctx* ctx, const float* d_xy, const int32_t* d_event_offs
  * the caller synchronises `stream`.  h_kept_xy / h_kept_idx NULL = lean mode:
  * only mask, peaks and counts come back (a host consumer that still holds h_xy
  * can compact by the mask).  Only the entries hough_run defines are meaningful;
- * the rest of h_peaks and of the kept arrays is zero.  NOT re-entrant (the
- * staging area belongs to the handle) and may allocate when a batch is larger
- * than any before. */
+ * the rest of h_peaks and of the kept arrays is zero.
+ *   The hit arrays (h_xy, h_keep_mask, h_kept_xy, h_kept_idx) are indexed by the
+ * offsets themselves: a SUB-BATCH of a larger host array passes the same array
+ * pointers with h_event_offsets advanced to its first event, and only its own
+ * hits h_event_offsets[0] .. h_event_offsets[n_events]-1 are copied; h_peaks and
+ * h_counts belong to the sub-batch ([n_events][...]).  The library keeps one
+ * device staging area per stream (up to 8 streams at a time, grow-only), so
+ * sub-batches issued on different streams overlap their host-to-device copy,
+ * kernel and device-to-host copies.
+ * Calls on ONE stream must not overlap in time from several host threads. */
 int hough_run_host(hough_ctx* ctx, const float* h_xy, const int32_t* h_event_offsets, int n_events,
                    uint8_t* h_keep_mask, hough_peak* h_peaks, int32_t* h_counts,
                    float* h_kept_xy, int32_t* h_kept_idx, hough_stream stream);

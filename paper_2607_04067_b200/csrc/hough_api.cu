@@ -51,6 +51,27 @@ struct Plan {
 
 }  // namespace
 
+// Device staging area of hough_run_host for one stream.
+struct Staging {
+    bool used = false;
+    cudaStream_t stream = nullptr;
+    unsigned long long tick = 0;
+    long long cap_hits = 0, cap_peaks = 0;
+    int cap_events = 0;
+    float* xy = nullptr;
+    int32_t* off = nullptr;
+    uint8_t* keep = nullptr;
+    hough_peak* peaks = nullptr;
+    int32_t* counts = nullptr;
+    float* kept_xy = nullptr;
+    int32_t* kept_idx = nullptr;
+    void release() {
+        cudaFree(xy); cudaFree(off); cudaFree(keep); cudaFree(peaks); cudaFree(counts); cudaFree(kept_xy); cudaFree(kept_idx);
+        xy = nullptr; off = nullptr; keep = nullptr; peaks = nullptr; counts = nullptr; kept_xy = nullptr; kept_idx = nullptr;
+        cap_hits = 0; cap_peaks = 0; cap_events = 0;
+    }
+};
+
 struct hough_ctx {
     int n_theta, n_rho, threshold, window;
     float rho_max, inv;
@@ -71,17 +92,10 @@ struct hough_ctx {
     float tmin_nz = 1.0f;    // smallest non-zero magnitude in the trig table
     Plan plan;
     std::atomic<long long> launches{0};
-    // hough_run_host staging (grow-only)
-    long long cap_hits = 0;
-    int cap_events = 0;
-    long long cap_peaks = 0;
-    float* s_xy = nullptr;
-    int32_t* s_off = nullptr;
-    uint8_t* s_keep = nullptr;
-    hough_peak* s_peaks = nullptr;
-    int32_t* s_counts = nullptr;
-    float* s_kept_xy = nullptr;
-    int32_t* s_kept_idx = nullptr;
+    // hough_run_host staging: one grow-only device area per stream (up to 8 streams at a time)
+    Staging staging[8];
+    unsigned long long staging_tick = 0;
+    std::mutex staging_mu;
 };
 
 namespace {
@@ -547,57 +561,69 @@ int hough_run_host(hough_ctx* c, const float* h_xy, const int32_t* h_off, int n_
     if (n_events < 0) return fail(HOUGH_ERR_INVALID_ARG, "n_events < 0");
     if (n_events == 0) return HOUGH_OK;
     if (!h_off || !h_keep || !h_counts || (!h_peaks && c->max_peaks > 0)) return fail(HOUGH_ERR_INVALID_ARG, "null host pointer");
-    const long long n_total = (long long)h_off[n_events] ;
-    if (n_total < 0 || (n_total > 0 && !h_xy)) return fail(HOUGH_ERR_INVALID_ARG, "bad offsets or null h_xy");
+    // the hit arrays are indexed by the offsets themselves: a sub-batch passes the same h_xy / h_keep with h_off advanced
+    const long long base = (long long)h_off[0], n_sub = (long long)h_off[n_events] - base;
+    if (base < 0 || n_sub < 0 || (n_sub > 0 && !h_xy)) return fail(HOUGH_ERR_INVALID_ARG, "bad offsets or null h_xy");
     cudaStream_t st = (cudaStream_t)stream;
     const long long n_peaks_cap = (long long)n_events * c->max_peaks;
-    if (n_total > c->cap_hits || n_events > c->cap_events || n_peaks_cap > c->cap_peaks) {
-        CUDA_TRY(cudaDeviceSynchronize());   // earlier copies on ANY stream may still use the old staging area
-        cudaFree(c->s_xy); cudaFree(c->s_off); cudaFree(c->s_keep); cudaFree(c->s_peaks); cudaFree(c->s_counts);
-        cudaFree(c->s_kept_xy); cudaFree(c->s_kept_idx);
-        c->s_xy = nullptr; c->s_off = nullptr; c->s_keep = nullptr; c->s_peaks = nullptr; c->s_counts = nullptr;
-        c->s_kept_xy = nullptr; c->s_kept_idx = nullptr;
-        c->cap_hits = std::max<long long>(n_total, c->cap_hits) + 16;
-        c->cap_events = std::max(n_events, c->cap_events);
-        c->cap_peaks = std::max<long long>(n_peaks_cap, c->cap_peaks) + 1;
-        cudaError_t e1 = cudaMalloc(&c->s_xy, sizeof(float) * 2 * c->cap_hits);
-        cudaError_t e2 = cudaMalloc(&c->s_off, sizeof(int32_t) * ((size_t)c->cap_events + 1));
-        cudaError_t e3 = cudaMalloc(&c->s_keep, (size_t)c->cap_hits);
-        cudaError_t e4 = cudaMalloc(&c->s_peaks, sizeof(hough_peak) * (size_t)c->cap_peaks);
-        cudaError_t e5 = cudaMalloc(&c->s_counts, sizeof(int32_t) * 2 * (size_t)c->cap_events);
-        cudaError_t e6 = cudaMalloc(&c->s_kept_xy, sizeof(float) * 2 * c->cap_hits);
-        cudaError_t e7 = cudaMalloc(&c->s_kept_idx, sizeof(int32_t) * c->cap_hits);
+
+    // one staging area per stream (N4c: streams + pinned memory + asynchronous transfers): calls on
+    // different streams overlap their H2D copy, kernel and D2H copies
+    Staging* sg = nullptr;
+    {
+        std::lock_guard<std::mutex> lk(c->staging_mu);
+        for (auto& x : c->staging) if (x.used && x.stream == st) sg = &x;
+        if (!sg) for (auto& x : c->staging) if (!x.used) { sg = &x; break; }
+        if (!sg) {                                    // all slots taken: recycle the least recently used one
+            sg = &c->staging[0];
+            for (auto& x : c->staging) if (x.tick < sg->tick) sg = &x;
+            CUDA_TRY(cudaStreamSynchronize(sg->stream));
+        }
+        sg->used = true; sg->stream = st; sg->tick = ++c->staging_tick;
+    }
+    if (n_sub > sg->cap_hits || n_events > sg->cap_events || n_peaks_cap > sg->cap_peaks) {
+        CUDA_TRY(cudaStreamSynchronize(st));          // the slot's earlier work runs on this very stream
+        sg->release();
+        sg->cap_hits = n_sub + 16; sg->cap_events = n_events; sg->cap_peaks = n_peaks_cap + 1;
+        cudaError_t e1 = cudaMalloc(&sg->xy, sizeof(float) * 2 * sg->cap_hits);
+        cudaError_t e2 = cudaMalloc(&sg->off, sizeof(int32_t) * ((size_t)sg->cap_events + 1));
+        cudaError_t e3 = cudaMalloc(&sg->keep, (size_t)sg->cap_hits);
+        cudaError_t e4 = cudaMalloc(&sg->peaks, sizeof(hough_peak) * (size_t)sg->cap_peaks);
+        cudaError_t e5 = cudaMalloc(&sg->counts, sizeof(int32_t) * 2 * (size_t)sg->cap_events);
+        cudaError_t e6 = cudaMalloc(&sg->kept_xy, sizeof(float) * 2 * sg->cap_hits);
+        cudaError_t e7 = cudaMalloc(&sg->kept_idx, sizeof(int32_t) * sg->cap_hits);
         if (e1 || e2 || e3 || e4 || e5 || e6 || e7) {
-            c->cap_hits = 0; c->cap_events = 0; c->cap_peaks = 0;
+            sg->release();
             return fail(HOUGH_ERR_NOMEM, "cudaMalloc of the staging area failed");
         }
     }
     // the kernel leaves peak entries past n_stored and kept entries past n_kept untouched: zero what goes back
-    if (c->max_peaks > 0) CUDA_TRY(cudaMemsetAsync(c->s_peaks, 0, sizeof(hough_peak) * (size_t)n_peaks_cap, st));
-    if (h_kept_xy && n_total > 0) CUDA_TRY(cudaMemsetAsync(c->s_kept_xy, 0, sizeof(float) * 2 * n_total, st));
-    if (h_kept_idx && n_total > 0) CUDA_TRY(cudaMemsetAsync(c->s_kept_idx, 0, sizeof(int32_t) * n_total, st));
-    if (n_total > 0) CUDA_TRY(cudaMemcpyAsync(c->s_xy, h_xy, sizeof(float) * 2 * n_total, cudaMemcpyHostToDevice, st));
-    CUDA_TRY(cudaMemcpyAsync(c->s_off, h_off, sizeof(int32_t) * ((size_t)n_events + 1), cudaMemcpyHostToDevice, st));
+    if (c->max_peaks > 0) CUDA_TRY(cudaMemsetAsync(sg->peaks, 0, sizeof(hough_peak) * (size_t)n_peaks_cap, st));
+    if (h_kept_xy && n_sub > 0) CUDA_TRY(cudaMemsetAsync(sg->kept_xy, 0, sizeof(float) * 2 * n_sub, st));
+    if (h_kept_idx && n_sub > 0) CUDA_TRY(cudaMemsetAsync(sg->kept_idx, 0, sizeof(int32_t) * n_sub, st));
+    if (n_sub > 0) CUDA_TRY(cudaMemcpyAsync(sg->xy, h_xy + 2 * base, sizeof(float) * 2 * n_sub, cudaMemcpyHostToDevice, st));
+    CUDA_TRY(cudaMemcpyAsync(sg->off, h_off, sizeof(int32_t) * ((size_t)n_events + 1), cudaMemcpyHostToDevice, st));
+    // The staged hit arrays hold hits base .. base+n_sub-1 at positions 0 ..; the kernel indexes them by the (absolute)
+    // offsets, so it is handed pointers moved back by `base` -- dereferenced only at base and beyond.
     hough_io io{};
-    io.d_xy = c->s_xy; io.d_event_offsets = c->s_off; io.n_events = n_events;
-    io.d_keep_mask = c->s_keep; io.d_peaks = c->s_peaks; io.d_counts = c->s_counts;
-    io.d_kept_xy = h_kept_xy ? c->s_kept_xy : nullptr;
-    io.d_kept_idx = h_kept_idx ? c->s_kept_idx : nullptr;
+    io.d_xy = sg->xy - 2 * base; io.d_event_offsets = sg->off; io.n_events = n_events;
+    io.d_keep_mask = sg->keep - base; io.d_peaks = sg->peaks; io.d_counts = sg->counts;
+    io.d_kept_xy = h_kept_xy ? sg->kept_xy - 2 * base : nullptr;
+    io.d_kept_idx = h_kept_idx ? sg->kept_idx - base : nullptr;
     int rc = launch(c, &io, st);
     if (rc != HOUGH_OK) return rc;
-    if (n_total > 0) CUDA_TRY(cudaMemcpyAsync(h_keep, c->s_keep, (size_t)n_total, cudaMemcpyDeviceToHost, st));
-    if (c->max_peaks > 0) CUDA_TRY(cudaMemcpyAsync(h_peaks, c->s_peaks, sizeof(hough_peak) * (size_t)n_peaks_cap, cudaMemcpyDeviceToHost, st));
-    CUDA_TRY(cudaMemcpyAsync(h_counts, c->s_counts, sizeof(int32_t) * 2 * (size_t)n_events, cudaMemcpyDeviceToHost, st));
-    if (h_kept_xy && n_total > 0) CUDA_TRY(cudaMemcpyAsync(h_kept_xy, c->s_kept_xy, sizeof(float) * 2 * n_total, cudaMemcpyDeviceToHost, st));
-    if (h_kept_idx && n_total > 0) CUDA_TRY(cudaMemcpyAsync(h_kept_idx, c->s_kept_idx, sizeof(int32_t) * n_total, cudaMemcpyDeviceToHost, st));
+    if (n_sub > 0) CUDA_TRY(cudaMemcpyAsync(h_keep + base, sg->keep, (size_t)n_sub, cudaMemcpyDeviceToHost, st));
+    if (c->max_peaks > 0) CUDA_TRY(cudaMemcpyAsync(h_peaks, sg->peaks, sizeof(hough_peak) * (size_t)n_peaks_cap, cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(cudaMemcpyAsync(h_counts, sg->counts, sizeof(int32_t) * 2 * (size_t)n_events, cudaMemcpyDeviceToHost, st));
+    if (h_kept_xy && n_sub > 0) CUDA_TRY(cudaMemcpyAsync(h_kept_xy + 2 * base, sg->kept_xy, sizeof(float) * 2 * n_sub, cudaMemcpyDeviceToHost, st));
+    if (h_kept_idx && n_sub > 0) CUDA_TRY(cudaMemcpyAsync(h_kept_idx + base, sg->kept_idx, sizeof(int32_t) * n_sub, cudaMemcpyDeviceToHost, st));
     return HOUGH_OK;
 }
 
 void hough_destroy(hough_ctx* c) {
     if (!c) return;
     cudaFree(c->d_cos); cudaFree(c->d_sin);
-    cudaFree(c->s_xy); cudaFree(c->s_off); cudaFree(c->s_keep); cudaFree(c->s_peaks); cudaFree(c->s_counts);
-    cudaFree(c->s_kept_xy); cudaFree(c->s_kept_idx);
+    for (auto& x : c->staging) x.release();
     delete c;
 }
 

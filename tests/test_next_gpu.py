@@ -179,3 +179,40 @@ def test_option_validation(hb):
     with pytest.raises(hb.HoughError):
         hb.hough_set_option_f64(h.ctx, 99, 1.0)
     h.close()
+
+
+# ---------------------------------------------------------------- N4c: sub-batches on several streams, one staging area each
+def test_n4c_host_sub_batches_on_several_streams_overlap_safely(hb):
+    import torch
+    w = si.config(1)
+    xy, off, _ = si.generate(w, 200)
+    table = si.trig_table(w.n_theta)
+    o = oracle.run(xy, off, w.n_theta, w.n_rho, w.rho_max, w.threshold, w.window, table[0], table[1], max_peaks=w.max_peaks, n_threads=8)
+    h = hb.Hough(w.n_theta, w.n_rho, w.rho_max, w.threshold, w.window, trig_table=table)
+    h_xy, h_off = torch.from_numpy(xy).pin_memory(), torch.from_numpy(off).pin_memory()
+    keep = torch.full((len(xy),), 9, dtype=torch.uint8).pin_memory()
+    peaks = torch.zeros((200, 64, 2), dtype=torch.int32).pin_memory()
+    counts = torch.full((200, 2), -7, dtype=torch.int32).pin_memory()
+    kxy = torch.zeros((len(xy), 2), dtype=torch.float32).pin_memory()
+    kidx = torch.full((len(xy),), -3, dtype=torch.int32).pin_memory()
+    streams = [torch.cuda.Stream() for _ in range(4)]
+    for rep in range(2):                                   # the second pass reuses every stream's staging area
+        for b, e0 in enumerate(range(0, 200, 25)):         # 8 sub-batches of 25 events, round-robin on 4 streams
+            hb.hough_run_host(h.ctx, h_xy, h_off[e0:], 25, keep, peaks[e0:], counts[e0:], kxy, kidx, stream=streams[b % 4])
+        torch.cuda.synchronize()
+        assert np.array_equal(counts.numpy(), o.counts) and np.array_equal(keep.numpy(), o.keep)
+        p3 = hb.unpack_peaks(peaks.numpy())
+        for e in range(200):
+            ns = min(int(o.counts[e, 0]), 64)
+            assert np.array_equal(p3[e, :ns], o.peaks[e, :ns]) and not p3[e, ns:].any()
+            nk, a = int(o.counts[e, 1]), int(off[e])
+            assert np.array_equal(kidx.numpy()[a:a + nk], o.kept_idx[a:a + nk])
+            assert np.array_equal(kxy.numpy()[a:a + nk].view(np.uint32), o.kept_xy[a:a + nk].view(np.uint32))
+            assert not kidx.numpy()[a + nk:int(off[e + 1])].any()          # the tail comes back zeroed
+    # more streams than staging slots: the least recently used slot is recycled
+    many = [torch.cuda.Stream() for _ in range(10)]
+    for b, e0 in enumerate(range(0, 200, 20)):
+        hb.hough_run_host(h.ctx, h_xy, h_off[e0:], 20, keep, peaks[e0:], counts[e0:], None, None, stream=many[b])
+    torch.cuda.synchronize()
+    assert np.array_equal(counts.numpy(), o.counts) and np.array_equal(keep.numpy(), o.keep)
+    h.close()

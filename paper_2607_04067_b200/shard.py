@@ -16,19 +16,6 @@ def event_range(rank: int, world: int, events_per_rank: int):
     return first, first + events_per_rank
 
 
-def split_events(n_events: int, world: int):
-    """Strong scaling: contiguous, balanced [begin, end) event ranges of one fixed batch, one per rank."""
-    if world < 1 or n_events < 0:
-        raise ValueError("bad n_events/world")
-    base, rem = divmod(n_events, world)
-    out, b = [], 0
-    for r in range(world):
-        e = b + base + (1 if r < rem else 0)
-        out.append((b, e))
-        b = e
-    return out
-
-
 def max_over_ranks(values, device=None):
     """Element-wise MAX of a list of floats over all ranks (identity when not initialised)."""
     import torch

@@ -59,11 +59,7 @@ def test_two_ranks_own_disjoint_event_ranges_and_reduce_by_max():
         assert abs(r[6] - 10 / 0.015) < 1e-6
 
 
-def test_split_events_is_a_balanced_partition():
-    for n, wld in ((1000, 8), (7, 3), (0, 4), (5, 8)):
-        parts = shard.split_events(n, wld)
-        assert parts[0][0] == 0 and parts[-1][1] == n
-        assert all(a[1] == b[0] for a, b in zip(parts, parts[1:]))
-        sizes = [e - b for b, e in parts]
-        assert max(sizes) - min(sizes) <= 1
+def test_event_ranges_of_the_ranks_tile_the_event_stream():
     assert shard.event_range(3, 4, 250) == (750, 1000)
+    ranges = [shard.event_range(r, 8, 125) for r in range(8)]
+    assert ranges[0][0] == 0 and all(a[1] == b[0] for a, b in zip(ranges, ranges[1:])) and ranges[-1][1] == 1000

@@ -1,6 +1,7 @@
 // hough_api.cu -- the C ABI of include/hough.h: handle management, shared-memory
 // planning, launch.  All compute is in hough_kernel.cuh; nothing here falls
 // back to the CPU.
+#include <algorithm>
 #include <atomic>
 #include <cmath>
 #include <cstdarg>
@@ -143,15 +144,11 @@ int prepare_kernel(int device, const void* fn, int smem_bytes, int csize) {
     return HOUGH_OK;
 }
 
-// Lays out shared memory for cluster size C and `want_ctas` CTAs per SM.  Returns false if it does not fit.
-bool try_plan(const hough_ctx* c, bool acc16, int C, int want_ctas, Plan* out) {
+// Lays out shared memory for cluster size C, `want_ctas` CTAs per SM and `cpl` theta columns per lane.  Returns false if
+// it does not fit or an invariant of the kernel's address arithmetic cannot be met.
+bool try_plan_cpl(const hough_ctx* c, bool acc16, int C, int want_ctas, int cpl, Plan* out) {
     const int cols = (c->n_theta + C - 1) / C;
-    // columns per lane: the choice that pads the fewest columns, ties to the larger (fewer broadcast loads per vote)
-    int cpl = 2, padded = 1 << 30;
-    for (int cand = 6; cand >= 2; cand -= 2) {
-        const int pc = (cols + 32 * cand - 1) / (32 * cand) * (32 * cand);
-        if (pc < padded) { padded = pc; cpl = cand; }
-    }
+    const int padded = (cols + 32 * cpl - 1) / (32 * cpl) * (32 * cpl);
     const int n_groups = padded / (32 * cpl);
     const int max_warps = want_ctas >= 2 ? 16 : 32;
     if (n_groups > max_warps) return false;
@@ -163,7 +160,8 @@ bool try_plan(const hough_ctx* c, bool acc16, int C, int want_ctas, Plan* out) {
     {
         const unsigned nan_rel = (0x7FFFFFFFu - HOUGH_MAGIC_BITS) * (unsigned)pitch_b;
         const unsigned long long end = (unsigned long long)(c->n_rho + 1) * (unsigned)pitch_b;
-        if ((unsigned long long)nan_rel < end || (unsigned long long)nan_rel + (unsigned)pitch_b > 0xFFFFFFFFull) return false;
+        // (the largest lane offset added to it is pitch - 4: no 32-bit wrap back into the accumulator)
+        if ((unsigned long long)nan_rel < end || (unsigned long long)nan_rel + (unsigned)pitch_b - 4ull > 0xFFFFFFFFull) return false;
     }
     const int wpr = (c->n_rho + 31) / 32;
     const int n_stripes = max_warps / n_groups;
@@ -223,6 +221,18 @@ bool try_plan(const hough_ctx* c, bool acc16, int C, int want_ctas, Plan* out) {
     out->smem_bytes = kp.misc_off + (int)misc_bytes;
     out->kp = kp;
     return true;
+}
+
+// Columns per lane: the choice that pads the fewest columns first, ties to the larger (fewer broadcast loads per
+// vote); a choice whose row pitch breaks an address invariant (e.g. the NaN rule above) falls through to the next.
+bool try_plan(const hough_ctx* c, bool acc16, int C, int want_ctas, Plan* out) {
+    const int cols = (c->n_theta + C - 1) / C;
+    int order[3] = {6, 4, 2};
+    auto padded = [&](int cand) { return (cols + 32 * cand - 1) / (32 * cand) * (32 * cand); };
+    std::stable_sort(order, order + 3, [&](int x, int y) { return padded(x) < padded(y); });   // ties keep the larger first
+    for (int a = 0; a < 3; ++a)
+        if (try_plan_cpl(c, acc16, C, want_ctas, order[a], out)) return true;
+    return false;
 }
 
 // Pure host logic (no CUDA call): the smallest cluster of {1,2,4,8} CTAs whose layout fits, two CTAs per SM if possible.

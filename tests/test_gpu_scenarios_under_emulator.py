@@ -77,7 +77,8 @@ PARITY = [
     ("test_conformal_scale_2", ()),
     ("test_default_trig_table_equals_harness_table", ()),
     ("test_p1_closed_form_on_gpu", ()),
-]
+    ("test_power_of_two_row_pitch_grid", ()),
+] + [("test_every_kernel_instantiation", inst) for inst in tp.INSTANTIATIONS]
 
 NEXT = [
     ("test_n1_circles_match_the_oracle_bit_for_bit", (2, 3)),

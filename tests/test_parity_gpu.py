@@ -265,6 +265,36 @@ def test_conformal_scale_2(hb):
         assert np.array_equal(g1[k], g2[k]), k          # pin P5 on the GPU
 
 
+# (acc, cluster, n_theta) -> one grid per kernel instantiation <ACC16, CL, CPL> (n_rho = 96); the
+# <u32, CL, 6> instantiation was never exercised
+INSTANTIATIONS = [("u16", 1, 40, 2), ("u16", 1, 100, 4), ("u16", 1, 180, 6), ("u16", 2, 100, 2), ("u16", 2, 200, 4), ("u16", 2, 360, 6),
+                  ("u32", 1, 40, 2), ("u32", 1, 100, 4), ("u32", 1, 180, 6), ("u32", 2, 100, 2), ("u32", 2, 200, 4), ("u32", 2, 360, 6)]
+
+
+@pytest.mark.parametrize("acc,cluster,n_theta,cpl", INSTANTIATIONS)
+def test_every_kernel_instantiation(hb, acc, cluster, n_theta, cpl):
+    plan = hb.hough_plan_describe(n_theta, 96, hb.HOUGH_ACC_U32 if acc == "u32" else hb.HOUGH_ACC_U16, cluster_size=cluster)
+    assert (plan["cols_per_lane"], plan["cluster_size"], plan["acc_bits"]) == (cpl, cluster, 32 if acc == "u32" else 16)
+    w = si.config(0)
+    xy, off, _ = si.generate(w, 3)
+    table = si.trig_table(n_theta)
+    g = gpu_run(hb, xy, off, n_theta, 96, w.rho_max, 14, 1, table, max_peaks=128, acc_dtype=acc, cluster_size=cluster)
+    o = oracle.run(xy, off, n_theta, 96, w.rho_max, 14, 1, table[0], table[1], max_peaks=128, acc_u16=(acc != "u32"), want_accum=True)
+    compare(g, o, off, 128, tag="%s C%d %d" % (acc, cluster, n_theta))
+    assert o.counts[:, 0].min() >= 1
+
+
+def test_power_of_two_row_pitch_grid(hb):
+    # 512 theta columns of u16 = 1024-byte rows: the canonical NaN of a padding column lands exactly one row short of
+    # the 32-bit wrap (tests/test_planner.py emulates it); round 1's planner refused this grid
+    w = si.config(0)
+    xy, off, _ = si.generate(w, 3)
+    table = si.trig_table(500)
+    g = gpu_run(hb, xy, off, 500, 96, w.rho_max, 14, 1, table, max_peaks=256)
+    o = oracle.run(xy, off, 500, 96, w.rho_max, 14, 1, table[0], table[1], max_peaks=256, want_accum=True)
+    compare(g, o, off, 256, tag="500x96")
+
+
 # ---------------------------------------------------------------- edge cases
 def test_empty_and_ragged_events(hb):
     w = si.config(0)

@@ -30,7 +30,7 @@ def check_plan(n_theta, n_rho, p):
     assert (1 << 17) * p["pitch_bytes"] < (1 << 31)
     # padding columns carry NaN table entries: their offset must fall beyond the accumulator for every word of a row
     nan_rel = ((0x7FFFFFFF - MAGIC_BITS) * p["pitch_bytes"]) & 0xFFFFFFFF
-    assert nan_rel >= (n_rho + 1) * p["pitch_bytes"] and nan_rel + p["pitch_bytes"] <= 0xFFFFFFFF
+    assert nan_rel >= (n_rho + 1) * p["pitch_bytes"] and nan_rel + p["pitch_bytes"] - 4 <= 0xFFFFFFFF   # largest lane offset: pitch - 4
     # regions follow each other, 16-byte aligned, and fit the CTA's shared memory
     assert p["pbm_off"] == p["region_bytes"]
     assert p["bitmap_words_per_row"] == (n_rho + 31) // 32

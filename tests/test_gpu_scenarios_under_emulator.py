@@ -1,4 +1,4 @@
-"""-m "not gpu": the scenarios of the `-m gpu` parity tests (tests/test_parity_gpu.py, tests/test_next_gpu.py), run
+"""-m "not gpu": the scenarios of the `-m gpu` parity tests (tests/test_parity_gpu.py, tests/test_parity_next_gpu.py), run
 through the SIMT emulator of tests/simt_emu with the bounds-checked flavour of the kernel source.  The GPU tests'
 own functions are called with their `gpu_run` / `gpu_ex` helper swapped for an emulator-backed one, so the inputs,
 options and assertions are exactly the ones the GPU will see.  This checks the kernel's logic and the design of those
@@ -9,7 +9,7 @@ import pytest
 import oracle
 import paper_2607_04067_b200 as hb
 import stcf_inputs as si
-import tests.test_next_gpu as tn
+import tests.test_parity_next_gpu as tn
 import tests.test_parity_gpu as tp
 from tests import simt_emu
 
@@ -58,6 +58,7 @@ def emulated(monkeypatch):
 
 
 PARITY = [
+    ("test_forced_cluster_of_eight_matches_oracle", ()),
     ("test_cluster_grid_360x512_u32_plans_eight_ctas", ()),
     ("test_cluster_with_degenerate_hits_takes_the_slow_path", (2,)),
     ("test_cluster_with_degenerate_hits_takes_the_slow_path", (8,)),

@@ -138,7 +138,12 @@ def test_n3_the_papers_1000x1000_grid_on_a_16_cta_cluster(hb):
     w = si.config(1)
     w = type(w)(**{**w.__dict__, "n_theta": 1000, "n_rho": 1000, "rho_max": 0.01, "threshold": 12, "window": 2, "max_peaks": 64})
     xy, off, _ = si.generate(w, 12)
-    g, o, _ = gpu_ex(hb, w, xy, off, conformal_scale=2, circles=True)
+    try:
+        g, o, _ = gpu_ex(hb, w, xy, off, conformal_scale=2, circles=True)
+    except hb.HoughError as e:
+        if "16-CTA cluster" in str(e):      # cudaOccupancyMaxActiveClusters: this device cannot host a non-portable cluster
+            pytest.skip(str(e))
+        raise
     assert g["info"]["CLUSTER_SIZE"] == 16 and o.counts[:, 0].min() >= 1
     gpu_ex(hb, w, xy, off, conformal_scale=2, theta_wrap=True, keep_mode=1, keep_tol=3.0, accum=False)
 

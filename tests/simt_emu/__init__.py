@@ -39,7 +39,8 @@ def build(debug_bounds: bool = False, force: bool = False) -> str:
 
 def run(xy, off, n_theta, n_rho, rho_max, threshold, window, table, max_peaks=64, acc_dtype="u16", accum=True,
         conformal_scale=1, cluster_size=0, ctas_per_sm=0, vote_path=0, grid_clusters=0, debug_bounds=False, timeout=900,
-        peak_mode=0, rel_permille=500, nms_radius=1, theta_wrap=False, keep_mode=0, keep_tol=0.0, b_field=1.0, circles=False):
+        peak_mode=0, rel_permille=500, nms_radius=1, theta_wrap=False, keep_mode=0, keep_tol=0.0, b_field=1.0, circles=False,
+        order=None):
     """Same arguments and result keys as tests/test_parity_gpu.py::gpu_run."""
     import paper_2607_04067_b200 as hb
     xy = np.ascontiguousarray(xy, dtype=np.float32).reshape(-1, 2)
@@ -66,7 +67,12 @@ def run(xy, off, n_theta, n_rho, rho_max, threshold, window, table, max_peaks=64
             f.write(struct.pack("<5f", rho_max32, float(inv), float(conformal_scale), tame, ftz_min))
             f.write(struct.pack("<2d", float(keep_tol), float(b_field)))
             f.write(c.tobytes()); f.write(s.tobytes()); f.write(off.tobytes()); f.write(xy.tobytes())
-        r = subprocess.run([build(debug_bounds), fin, fout], capture_output=True, text=True, timeout=timeout)
+        env = dict(os.environ)
+        if order:                      # fiber scheduling order: "reverse", "shuffle:<seed>" (simt_shim.h run_cluster)
+            env["HOUGH_EMU_ORDER"] = order
+        else:
+            env.pop("HOUGH_EMU_ORDER", None)
+        r = subprocess.run([build(debug_bounds), fin, fout], capture_output=True, text=True, timeout=timeout, env=env)
         if r.returncode != 0:
             raise RuntimeError("hough_emu failed (rc %d): %s" % (r.returncode, r.stderr.strip()[-400:]))
         raw = open(fout, "rb").read()

@@ -14,6 +14,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <utility>
 #include <vector>
 
 #define __global__
@@ -188,12 +189,27 @@ inline void run_cluster(int cluster, int n_clusters, int csize, int threads, siz
             makecontext(&f.ctx, (void (*)())fiber_main, 0);
         }
     }
+    // Order in which the fibers get their turn in every scheduling pass.  A fiber runs until its next barrier or warp
+    // collective, so the order decides which thread's phase runs first: code that is missing a barrier between a producer
+    // and a consumer gives different results under different orders.  HOUGH_EMU_ORDER = forward (default) | reverse |
+    // shuffle[:seed] (a fresh pseudo-random permutation per pass).
+    const char* ord = getenv("HOUGH_EMU_ORDER");
+    const bool reverse = ord && !strncmp(ord, "reverse", 7), shuffle = ord && !strncmp(ord, "shuffle", 7);
+    unsigned long long rng = 0x9E3779B97F4A7C15ull ^ (shuffle && ord[7] == ':' ? strtoull(ord + 8, nullptr, 10) : 0ull) ^ (unsigned)cluster;
+    std::vector<size_t> order(fibers.size());
+    for (size_t i = 0; i < order.size(); ++i) order[i] = reverse ? order.size() - 1 - i : i;
     size_t live = fibers.size();
     while (live) {
         unsigned long before = 0, after = 0;
         for (auto& f : fibers) before += f.progress;
         size_t finished_now = 0;
-        for (auto& f : fibers) {
+        if (shuffle)
+            for (size_t i = order.size() - 1; i > 0; --i) {
+                rng = rng * 6364136223846793005ull + 1442695040888963407ull;
+                std::swap(order[i], order[(size_t)((rng >> 33) % (i + 1))]);
+            }
+        for (size_t oi = 0; oi < order.size(); ++oi) {
+            Fiber& f = fibers[order[oi]];
             if (f.done) continue;
             cur = &f;
             swapcontext(&g.sched, &f.ctx);

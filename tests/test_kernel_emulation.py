@@ -15,7 +15,7 @@ def emu_both(w, xy, off, accum=True, **kw):
     table = si.trig_table(w.n_theta)
     args = dict(max_peaks=w.max_peaks, acc_dtype=w.acc_dtype, threshold=w.threshold, window=w.window)
     args.update(kw)
-    emu_only = {k: args.pop(k) for k in ("cluster_size", "ctas_per_sm", "vote_path", "grid_clusters", "debug_bounds") if k in args}
+    emu_only = {k: args.pop(k) for k in ("cluster_size", "ctas_per_sm", "vote_path", "grid_clusters", "debug_bounds", "order") if k in args}
     g = simt_emu.run(xy, off, w.n_theta, w.n_rho, w.rho_max, args["threshold"], args["window"], table,
                      max_peaks=args["max_peaks"], acc_dtype=args["acc_dtype"], accum=accum,
                      conformal_scale=args.get("conformal_scale", 1), **emu_only)
@@ -150,3 +150,22 @@ def test_n3_the_papers_1000x1000_grid_under_the_emulator():
     xy, off, _ = si.generate(w, 1)
     g, o = emu_ex(w, xy, off, conformal_scale=2, debug_bounds=True, accum=True)
     assert g["info"]["CLUSTER_SIZE"] == 16 and o.counts[0, 0] >= 2
+
+
+# ---------------------------------------------------------------- scheduling-order independence (a weak synccheck)
+@pytest.mark.parametrize("order", ["reverse", "shuffle:1", "shuffle:2"])
+def test_results_do_not_depend_on_the_order_in_which_threads_reach_their_barriers(order):
+    # a fiber runs until its next barrier / warp collective; a phase that reads what another thread has not yet written
+    # (a missing barrier) gives different results when the threads take their turns in another order
+    w = si.config(0)
+    xy, off, _ = si.generate(w, 2)
+    emu_both(w, xy, off, order=order)
+    emu_both(w, xy, off, cluster_size=2, order=order)
+    w1 = si.config(1)
+    xy1, off1, _ = si.generate(w1, 1)
+    emu_ex(w1, xy1, off1, peak_mode=1, rel_permille=300, nms_radius=2, circles=True, order=order)
+    emu_ex(w, xy, off, theta_wrap=True, keep_mode=1, keep_tol=5.0, cluster_size=2, order=order)
+    w3 = si.config(3)
+    xy3, off3, _ = si.generate(w3, 4)
+    big = np.ascontiguousarray(xy3[:off3[4]])          # ~11000 hits as one event: several staging chunks, several selection blocks
+    emu_both(w3, big, np.array([0, len(big)], dtype=np.int32), threshold=45, cluster_size=2, order=order)

@@ -66,7 +66,7 @@ typedef struct hough_circle {
 typedef enum hough_status {
     HOUGH_OK = 0,
     HOUGH_ERR_INVALID_ARG = -1,   /* null pointer, out-of-range value */
-    HOUGH_ERR_UNSUPPORTED = -2,   /* grid does not fit even a 16-CTA cluster's shared memory, or an option needs one CTA per event */
+    HOUGH_ERR_UNSUPPORTED = -2,   /* grid does not fit even a 16-CTA cluster's shared memory */
     HOUGH_ERR_CUDA = -3,          /* a CUDA call failed (no device, launch error, ...) */
     HOUGH_ERR_NOMEM = -4          /* host or device allocation failed */
 } hough_status;
@@ -86,7 +86,7 @@ typedef enum hough_option {
     HOUGH_OPT_PEAK_MODE = 7,        /* 0 = absolute threshold + 3x3 local maximum, raster order (default);
                                        1 = threshold relative to the event's global accumulator maximum + iterative
                                        "extract the most significant peak, suppress its neighbourhood":
-                                       peaks come out in extraction order; needs one CTA per event */
+                                       peaks come out in extraction order (descending votes) */
     HOUGH_OPT_REL_THRESHOLD_PERMILLE = 8,  /* peak mode 1: candidates need votes >= ceil(value * A_max / 1000) and >= threshold;
                                        0..1000, default 500 */
     HOUGH_OPT_NMS_RADIUS = 9,       /* peak mode 1: half-width in bins of the suppressed neighbourhood, 0..64 (default 1) */

@@ -355,8 +355,6 @@ int launch(hough_ctx* c, const hough_io* io, cudaStream_t stream) {
     kp.diag = c->opt_vote_path >= 2 ? c->opt_vote_path : 0;
 #endif
     const bool ext = wants_ext(c);
-    if (ext && c->peak_mode == 1 && pl.csize > 1)
-        return fail(HOUGH_ERR_UNSUPPORTED, "peak mode 1 (iterative NMS) needs the accumulator in one CTA; this grid takes a %d-CTA cluster", pl.csize);
     kp.peak_mode = c->peak_mode; kp.rel_permille = c->rel_permille; kp.nms_radius = c->nms_radius;
     kp.theta_wrap = c->theta_wrap; kp.keep_mode = c->keep_mode; kp.keep_tol = c->keep_tol;
     const int C = pl.csize;

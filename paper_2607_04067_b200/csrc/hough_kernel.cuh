@@ -422,12 +422,12 @@ __global__ void __launch_bounds__(1024, 1) hough_event_kernel(const __grid_const
         }
 
         int n_stored;
-        if (EXT && !CL && p.peak_mode == 1) {
+        if (EXT && p.peak_mode == 1) {
             // ---- N2: threshold relative to the global maximum + iterative "extract the most
-            // significant peak, suppress its neighbourhood" (reading Q18).  One CTA holds the whole
-            // accumulator.  rowkey[k] = best cell of rho row k as (votes << 32) | (0xFFFF - j) << 16 | (0xFFFF - k): the
-            // maximum over keys is the largest count and, among equals, the raster-first cell.  All warps build the row
-            // keys; warp 0 then runs the extraction loop alone (a few hundred cycles per peak: 2R+1 rows to refresh).
+            // significant peak, suppress its neighbourhood" (reading Q18).
+            // rowkey[k] = best cell of this CTA's columns in rho row k as (votes << 32) | (0xFFFF - j) << 16 | (0xFFFF - k):
+            // the maximum over keys is the largest count and, among equals, the raster-first cell.  All warps build the
+            // row keys; the extraction loop costs a few hundred cycles per peak (2R+1 rows to refresh).
             ull* rowkey = (ull*)pbm;      // the peak bitmap is unused in this mode; the planner sizes it for n_rho keys
             auto warp_max = [&](ull best) -> ull {
 #pragma unroll
@@ -452,62 +452,108 @@ __global__ void __launch_bounds__(1024, 1) hough_event_kernel(const __grid_const
                 if (lane == 0 && HB_CHK(8 * k + 8 <= p.pbm_bytes, HB_H4)) rowkey[k] = b;
             }
             __syncthreads();
-            if (warp == 0) {
-                auto global_best = [&]() -> ull {
-                    ull best = 0;
-                    for (int k = lane; k < p.n_rho; k += 32)
-                        if (HB_CHK(8 * k + 8 <= p.pbm_bytes, HB_H4)) { const ull b = rowkey[k]; if (b > best) best = b; }
-                    return warp_max(best);
-                };
-                ull best = global_best();
-                const ull rel = ((ull)p.rel_permille * (ull)(unsigned)(best >> 32) + 999ull) / 1000ull;
-                const ull thr_eff = (ull)p.threshold > rel ? (ull)p.threshold : rel;
-                const int R = p.nms_radius, side = 2 * R + 1;
-                int n_found = 0;
-                for (;;) {
+            auto local_best = [&]() -> ull {      // whole warp: best key over this CTA's rows
+                ull best = 0;
+                for (int k = lane; k < p.n_rho; k += 32)
+                    if (HB_CHK(8 * k + 8 <= p.pbm_bytes, HB_H4)) { const ull b = rowkey[k]; if (b > best) best = b; }
+                return warp_max(best);
+            };
+            const int R = p.nms_radius, side = 2 * R + 1;
+            // whole warp: zero the (2R+1)^2 neighbourhood of (j, k) -- the cells this CTA owns -- and refresh the keys of
+            // the rows that changed (and of their mirrors when the neighbourhood crosses the theta seam)
+            auto suppress = [&](int j, int k) {
+                for (int idx = lane; idx < side * side; idx += 32) {
+                    int jj = j + idx / side - R, kk = k + idx % side - R;
+                    if (kk < 0 || kk >= p.n_rho) continue;
+                    if (jj < 0 || jj >= p.n_theta) {
+                        if (!p.theta_wrap) continue;
+                        while (jj < 0) { jj += p.n_theta; kk = p.n_rho - 1 - kk; }
+                        while (jj >= p.n_theta) { jj -= p.n_theta; kk = p.n_rho - 1 - kk; }
+                    }
+                    const int jl = jj - col0;
+                    if (jl < 0 || jl >= ncols) continue;       // another CTA of the cluster owns this column
+                    const unsigned woff = (unsigned)kk * pitch + 4u * cell_word_off<ACC16>(jl);
+                    if (!HB_CHK(woff + 4 <= limit, HB_H4)) continue;
+                    const unsigned mask = ACC16 ? (0xFFFFu << (16 * ((jl >> 5) & 1))) : 0xFFFFFFFFu;
+                    atomicAnd((unsigned*)(acc + woff), ~mask);     // two columns share a u16 word: clear one half atomically
+                }
+                const bool seam = p.theta_wrap && (j - R < 0 || j + R >= p.n_theta);
+                __syncwarp();
+                for (int kk = k - R; kk <= k + R; ++kk) {
+                    if (kk < 0 || kk >= p.n_rho) continue;
+                    const ull b = row_best(kk);
+                    if (lane == 0) rowkey[kk] = b;
+                    if (seam) {
+                        const ull bm = row_best(p.n_rho - 1 - kk);
+                        if (lane == 0) rowkey[p.n_rho - 1 - kk] = bm;
+                    }
+                }
+                __syncwarp();
+            };
+            auto thr_of = [&](ull first_best) -> ull {      // reading Q18: max(threshold, ceil(permille * A_max / 1000))
+                const ull rel = ((ull)p.rel_permille * (ull)(unsigned)(first_best >> 32) + 999ull) / 1000ull;
+                return (ull)p.threshold > rel ? (ull)p.threshold : rel;
+            };
+            int n_found = 0;
+            if (!CL) {
+                // one CTA holds the whole accumulator: warp 0 runs the extraction loop alone, no block barrier per peak
+                if (warp == 0) {
+                    ull best = local_best();
+                    const ull thr_eff = thr_of(best);
+                    for (;;) {
+                        const unsigned a = (unsigned)(best >> 32);
+                        if (a == 0u || (ull)a < thr_eff) break;
+                        const int j = 0xFFFF - (int)((best >> 16) & 0xFFFFull), k = 0xFFFF - (int)(best & 0xFFFFull);
+                        if (lane == 0 && n_found < p.max_peaks) {
+                            hough_peak pk;
+                            pk.theta_bin = (uint16_t)j; pk.rho_bin = (uint16_t)k; pk.votes = a;
+                            p.peaks[(size_t)e * p.max_peaks + n_found] = pk;
+                        }
+                        ++n_found;
+                        suppress(j, k);
+                        best = local_best();
+                    }
+                    if (lane == 0) misc[43] = n_found;
+                }
+                __syncthreads();
+                n_found = misc[43];
+            } else {
+                // theta columns are split over the cluster: every iteration each CTA's warp 0 publishes its local best
+                // (double-buffered slot), one cluster.sync, every CTA reduces the C slots over DSMEM to the SAME global
+                // best and takes the same decision; each CTA suppresses the cells it owns.  One cluster barrier per peak.
+                ull* slot = (ull*)(misc + 44);      // [2] local best of this CTA, by iteration parity (remote-readable)
+                ull* gbest = (ull*)(misc + 48);     // [2] the cluster's best, by iteration parity
+                ull thr_eff = 0;
+                for (int it = 0;; ++it) {
+                    if (warp == 0) {
+                        const ull lb = local_best();
+                        if (lane == 0) slot[it & 1] = lb;
+                    }
+                    cg::this_cluster().sync();
+                    if (warp == 0) {
+                        ull v = 0;
+                        if (lane < C) v = *(const ull*)cg::this_cluster().map_shared_rank((void*)&slot[it & 1], lane);
+                        v = warp_max(v);
+                        if (lane == 0) gbest[it & 1] = v;
+                    }
+                    __syncthreads();
+                    const ull best = gbest[it & 1];
+                    if (it == 0) thr_eff = thr_of(best);
                     const unsigned a = (unsigned)(best >> 32);
-                    if (a == 0u || (ull)a < thr_eff) break;
+                    if (a == 0u || (ull)a < thr_eff) break;      // the same value in every thread of every CTA
                     const int j = 0xFFFF - (int)((best >> 16) & 0xFFFFull), k = 0xFFFF - (int)(best & 0xFFFFull);
-                    if (lane == 0 && n_found < p.max_peaks) {
+                    if (rank == 0 && tid == 0 && n_found < p.max_peaks) {
                         hough_peak pk;
                         pk.theta_bin = (uint16_t)j; pk.rho_bin = (uint16_t)k; pk.votes = a;
                         p.peaks[(size_t)e * p.max_peaks + n_found] = pk;
                     }
                     ++n_found;
-                    bool seam = false;            // does the neighbourhood cross the theta seam (then mirrored rows change too)
-                    for (int idx = lane; idx < side * side; idx += 32) {
-                        int jj = j + idx / side - R, kk = k + idx % side - R;
-                        if (kk < 0 || kk >= p.n_rho) continue;
-                        if (jj < 0 || jj >= p.n_theta) {
-                            if (!p.theta_wrap) continue;
-                            while (jj < 0) { jj += p.n_theta; kk = p.n_rho - 1 - kk; }
-                            while (jj >= p.n_theta) { jj -= p.n_theta; kk = p.n_rho - 1 - kk; }
-                        }
-                        const int jl = jj - col0;
-                        const unsigned woff = (unsigned)kk * pitch + 4u * cell_word_off<ACC16>(jl);
-                        if (!HB_CHK(jl >= 0 && jl < ncols && woff + 4 <= limit, HB_H4)) continue;
-                        const unsigned mask = ACC16 ? (0xFFFFu << (16 * ((jl >> 5) & 1))) : 0xFFFFFFFFu;
-                        atomicAnd((unsigned*)(acc + woff), ~mask);     // two columns share a u16 word: clear one half atomically
-                    }
-                    if (p.theta_wrap && (j - R < 0 || j + R >= p.n_theta)) seam = true;
-                    __syncwarp();
-                    for (int kk = k - R; kk <= k + R; ++kk) {
-                        if (kk < 0 || kk >= p.n_rho) continue;
-                        const ull b = row_best(kk);
-                        if (lane == 0) rowkey[kk] = b;
-                        if (seam) {
-                            const ull bm = row_best(p.n_rho - 1 - kk);
-                            if (lane == 0) rowkey[p.n_rho - 1 - kk] = bm;
-                        }
-                    }
-                    __syncwarp();
-                    best = global_best();
+                    if (warp == 0) suppress(j, k);
                 }
-                if (lane == 0) misc[43] = n_found;
+                __threadfence();
+                cg::this_cluster().sync();   // rank 0's stored peaks are visible cluster-wide; no CTA leaves while its slot may be read
             }
-            __syncthreads();
-            const int n_found = misc[43];
-            if (tid == 0) p.counts[2 * e] = n_found;
+            if (rank == 0 && tid == 0) p.counts[2 * e] = n_found;
             n_stored = min(n_found, p.max_peaks);
         } else {
         // ---- H4: threshold + 3x3 local maximum -> peak bitmap (reading Q8)

@@ -100,7 +100,6 @@ int main(int argc, char** argv) {
     kp.rcp_groups = (unsigned)plan[24]; kp.rcp_2s = (unsigned)plan[25]; kp.circ_cap = plan[26];
     kp.peak_mode = peak_mode; kp.rel_permille = rel_permille; kp.nms_radius = nms_radius; kp.theta_wrap = theta_wrap;
     kp.keep_mode = keep_mode; kp.keep_tol = dbl[0];
-    if (peak_mode == 1 && csize > 1) emu::die("peak mode 1 needs one CTA per event (hough_run refuses this too)");
     kp.vpr = kp.pitch_b / 16;
     if (plan[0] != csize || plan[1] != threads || plan[2] != smem_bytes || plan[4] != g_cpl || (plan[3] == 16) != (g_acc16 != 0))
         emu::die("header and plan disagree");

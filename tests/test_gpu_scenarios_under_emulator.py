@@ -31,10 +31,6 @@ def emu_gpu_ex(_hb, w, xy, off, accum=True, circles=False, cluster_size=0, rho_m
     opts = {k: kw.pop(k) for k in list(kw) if k in tn.OPTS}
     assert not kw, kw
     rho_max = w.rho_max if rho_max is None else rho_max
-    plan = hb.hough_plan_describe(w.n_theta, w.n_rho, {"u16": hb.HOUGH_ACC_U16, "u32": hb.HOUGH_ACC_U32}[base["acc_dtype"]],
-                                  cluster_size=cluster_size)
-    if opts.get("peak_mode") == 1 and plan["cluster_size"] > 1:      # what hough_run answers (hough_api.cu launch())
-        raise hb.HoughError("peak mode 1 (iterative NMS) needs the accumulator in one CTA")
     g = simt_emu.run(xy, off, w.n_theta, w.n_rho, rho_max, base["threshold"], base["window"], table, max_peaks=base["max_peaks"],
                      acc_dtype=base["acc_dtype"], accum=accum, conformal_scale=base["conformal_scale"], circles=circles,
                      cluster_size=cluster_size, debug_bounds=True, **opts)
@@ -95,6 +91,7 @@ NEXT = [
     ("test_n4b_distance_filter", (1, 6, 4, 20.0)),
     ("test_n4b_distance_filter", (3, 2, 0, 0.5)),
     ("test_n4b_more_stored_peaks_than_staged_circles", ()),
+    ("test_n2_with_theta_wrap_and_on_cluster_grids", ()),
 ]
 
 

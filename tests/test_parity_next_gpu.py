@@ -119,17 +119,23 @@ def test_n2_relative_threshold_and_iterative_nms(hb, cfg, n_ev, permille, radius
     gpu_ex(hb, w, xy, off, peak_mode=1, rel_permille=permille, nms_radius=radius, max_peaks=3, accum=False)     # truncation
 
 
-def test_n2_full_batch_and_wrap_and_refusal_on_cluster_grids(hb):
+def test_n2_full_batch_of_1000_events(hb):
     w = si.config(1)
-    xy, off, _ = si.generate(w)                                     # the 1000-event batch
+    xy, off, _ = si.generate(w)
     gpu_ex(hb, w, xy, off, peak_mode=1, rel_permille=500, nms_radius=2, accum=False)
+
+
+def test_n2_with_theta_wrap_and_on_cluster_grids(hb):
     w0 = si.config(0)
     xy, off = seam_events(w0, 4)
     gpu_ex(hb, w0, xy, off, peak_mode=1, rel_permille=300, nms_radius=2, theta_wrap=True, threshold=12)
+    # theta columns split over a cluster: one cluster barrier per extracted peak, the same decision in every CTA
     w5 = si.config(5)
-    xy, off, _ = si.generate(w5, 2)
-    with pytest.raises(hb.HoughError, match="one CTA"):
-        gpu_ex(hb, w5, xy, off, peak_mode=1)
+    xy, off, _ = si.generate(w5, 3)
+    gpu_ex(hb, w5, xy, off, peak_mode=1, rel_permille=400, nms_radius=2)
+    xy, off = seam_events(w0, 4)
+    for cluster in (2, 8):
+        gpu_ex(hb, w0, xy, off, peak_mode=1, rel_permille=300, nms_radius=3, theta_wrap=True, threshold=12, cluster_size=cluster, circles=True)
 
 
 # ---------------------------------------------------------------- N3
@@ -146,6 +152,8 @@ def test_n3_the_papers_1000x1000_grid_on_a_16_cta_cluster(hb):
         raise
     assert g["info"]["CLUSTER_SIZE"] == 16 and o.counts[:, 0].min() >= 1
     gpu_ex(hb, w, xy, off, conformal_scale=2, theta_wrap=True, keep_mode=1, keep_tol=3.0, accum=False)
+    # the paper's own peak finder on the paper's own grid
+    gpu_ex(hb, w, xy[:off[3]], off[:4], conformal_scale=2, peak_mode=1, rel_permille=500, nms_radius=3, theta_wrap=True, circles=True)
 
 
 # ---------------------------------------------------------------- N4a / N4b

@@ -92,9 +92,14 @@ typedef enum hough_option {
     HOUGH_OPT_NMS_RADIUS = 9,       /* peak mode 1: half-width in bins of the suppressed neighbourhood, 0..64 (default 1) */
     HOUGH_OPT_THETA_WRAP = 10,      /* 1 = (theta + pi, rho) == (theta, -rho): column -1 is column n_theta-1 with the rho
                                        index mirrored, for the 3x3 test, the suppression and the keep windows (default 0) */
-    HOUGH_OPT_KEEP_MODE = 11        /* 0 = (theta, rho) window around the stored peaks (default); 1 = original-space road
+    HOUGH_OPT_KEEP_MODE = 11,       /* 0 = (theta, rho) window around the stored peaks (default); 1 = original-space road
                                        | ||hit - centre|| - r_c | < HOUGH_OPTF_KEEP_TOL around their candidate circles
                                        ("inversely mapped back to the original space ... data filtering") */
+    HOUGH_OPT_STAGING = 12          /* how an event's hits reach shared memory (H0; PAPER.md:86 names non-coalesced access
+                                       as a hazard): 0 = coalesced float2 loads issued ahead of the zeroing stores (default);
+                                       1 = one cp.async.bulk (TMA engine) per chunk, completion on an mbarrier, the 16-byte
+                                       aligned source range found by aligning down and up by one hit; needs d_xy 16-byte
+                                       aligned.  Same results; never yet timed */
 } hough_option;
 
 typedef enum hough_option_f64 {

@@ -9,7 +9,8 @@
 
 The kernels use __fmul_rn/__fadd_rn/__fadd_rd and -fmad=false so that no multiply-add is ever contracted (DESIGN.md
 S2); as a belt-and-braces check the product's SASS must contain no packed FFMA2 and must contain the floor-add
-(FADD.RM), the clamp (VIMNMX) and the vote (ATOMS.POPC.INC)."""
+(FADD.RM), the clamp (VIMNMX) and the vote (ATOMS.POPC.INC); the bulk-copy staging option must show up as UBLKCP, and only
+in the extended instantiations."""
 import os
 import re
 import subprocess
@@ -56,9 +57,15 @@ def check_sass(lib: str = LIB) -> None:
     sass = _sass(lib)
     if "FFMA2" in sass:
         raise RuntimeError("ptxas contracted a packed fp32 multiply-add (FFMA2 found): bit-exactness is lost")
-    for needle in ("FADD.RM", "ATOMS.POPC.INC", "VIMNMX"):
+    for needle in ("FADD.RM", "ATOMS.POPC.INC", "VIMNMX", "UBLKCP"):
         if needle not in sass:
             raise RuntimeError("expected %s in the SASS of %s" % (needle, lib))
+    # the default instantiations (EXT = false, last template argument Lb0E) carry none of the optional paths:
+    # no bulk copy / mbarrier, no fp64 arithmetic of the distance filter
+    for m in re.finditer(r"Function : (\S*hough_event_kernelI\S*ELb0EEE\S*)\n(.*?)(?=\n\s*Function : |\Z)", sass, flags=re.S):
+        for needle in ("UBLKCP", "SYNCS", "DADD", "DMUL", "DFMA"):
+            if needle in m.group(2):
+                raise RuntimeError("%s found in the default instantiation %s" % (needle, m.group(1)))
 
 
 # hough_bench_issue_rate(kind): SASS opcodes that one loop trip of issue_kernel<kind> must hold, and how many

@@ -82,7 +82,7 @@ struct hough_ctx {
     int opt_cluster = 0;
     int opt_ctas_per_sm = 0;
     int opt_vote_path = 0;
-    int peak_mode = 0, rel_permille = 500, nms_radius = 1, theta_wrap = 0, keep_mode = 0;
+    int peak_mode = 0, rel_permille = 500, nms_radius = 1, theta_wrap = 0, keep_mode = 0, stage_mode = 0;
     double keep_tol = 0.0, b_field = 1.0;
     int device = 0;
     int sm_count = 0;
@@ -121,7 +121,7 @@ const void* pick_kernel(bool acc16, bool cl, int cpl, bool ext) {
     return cl ? kernel_ptr<false, true, false>(cpl) : kernel_ptr<false, false, false>(cpl);
 }
 
-bool wants_ext(const hough_ctx* c) { return c->peak_mode != 0 || c->theta_wrap != 0 || c->keep_mode != 0; }
+bool wants_ext(const hough_ctx* c) { return c->peak_mode != 0 || c->theta_wrap != 0 || c->keep_mode != 0 || c->stage_mode != 0; }
 
 // cudaFuncAttributeMaxDynamicSharedMemorySize belongs to the kernel (per device), not to a handle: several live
 // handles may share one instantiation with different footprints, so the attribute is only ever RAISED.
@@ -357,6 +357,9 @@ int launch(hough_ctx* c, const hough_io* io, cudaStream_t stream) {
     const bool ext = wants_ext(c);
     kp.peak_mode = c->peak_mode; kp.rel_permille = c->rel_permille; kp.nms_radius = c->nms_radius;
     kp.theta_wrap = c->theta_wrap; kp.keep_mode = c->keep_mode; kp.keep_tol = c->keep_tol;
+    kp.stage_mode = c->stage_mode;
+    if (c->stage_mode == 1 && ((uintptr_t)io->d_xy & 15u) != 0)
+        return fail(HOUGH_ERR_INVALID_ARG, "bulk-copy staging needs d_xy 16-byte aligned");
     const int C = pl.csize;
     // one CTA (cluster) per event: the hardware block scheduler deals events to the SM slots as they free up, which
     // balances events of different size; the kernel's event loop only matters beyond 2^31 CTAs
@@ -451,6 +454,9 @@ int hough_set_option(hough_ctx* c, int key, long long value) {
         case HOUGH_OPT_KEEP_MODE:
             if (value != 0 && value != 1) return fail(HOUGH_ERR_INVALID_ARG, "keep mode must be 0 or 1");
             c->keep_mode = (int)value; return HOUGH_OK;
+        case HOUGH_OPT_STAGING:
+            if (value != 0 && value != 1) return fail(HOUGH_ERR_INVALID_ARG, "staging must be 0 or 1");
+            c->stage_mode = (int)value; return HOUGH_OK;
         default: break;
     }
     switch (key) {
@@ -589,10 +595,10 @@ int hough_run_host(hough_ctx* c, const float* h_xy, const int32_t* h_off, int n_
         }
         sg->used = true; sg->stream = st; sg->tick = ++c->staging_tick;
     }
-    if (n_sub > sg->cap_hits || n_events > sg->cap_events || n_peaks_cap > sg->cap_peaks) {
+    if (n_sub + 1 > sg->cap_hits || n_events > sg->cap_events || n_peaks_cap > sg->cap_peaks) {
         CUDA_TRY(cudaStreamSynchronize(st));          // the slot's earlier work runs on this very stream
         sg->release();
-        sg->cap_hits = n_sub + 16; sg->cap_events = n_events; sg->cap_peaks = n_peaks_cap + 1;
+        sg->cap_hits = n_sub + 17; sg->cap_events = n_events; sg->cap_peaks = n_peaks_cap + 1;
         cudaError_t e1 = cudaMalloc(&sg->xy, sizeof(float) * 2 * sg->cap_hits);
         cudaError_t e2 = cudaMalloc(&sg->off, sizeof(int32_t) * ((size_t)sg->cap_events + 1));
         cudaError_t e3 = cudaMalloc(&sg->keep, (size_t)sg->cap_hits);
@@ -609,12 +615,15 @@ int hough_run_host(hough_ctx* c, const float* h_xy, const int32_t* h_off, int n_
     if (c->max_peaks > 0) CUDA_TRY(cudaMemsetAsync(sg->peaks, 0, sizeof(hough_peak) * (size_t)n_peaks_cap, st));
     if (h_kept_xy && n_sub > 0) CUDA_TRY(cudaMemsetAsync(sg->kept_xy, 0, sizeof(float) * 2 * n_sub, st));
     if (h_kept_idx && n_sub > 0) CUDA_TRY(cudaMemsetAsync(sg->kept_idx, 0, sizeof(int32_t) * n_sub, st));
-    if (n_sub > 0) CUDA_TRY(cudaMemcpyAsync(sg->xy, h_xy + 2 * base, sizeof(float) * 2 * n_sub, cudaMemcpyHostToDevice, st));
+    // hits keep the parity of their absolute index in the staging buffer (hit `base` goes to slot base & 1), so that the
+    // pointer handed to the kernel stays 16-byte aligned (bulk-copy staging relies on it)
+    const long long par = base & 1;
+    if (n_sub > 0) CUDA_TRY(cudaMemcpyAsync(sg->xy + 2 * par, h_xy + 2 * base, sizeof(float) * 2 * n_sub, cudaMemcpyHostToDevice, st));
     CUDA_TRY(cudaMemcpyAsync(sg->off, h_off, sizeof(int32_t) * ((size_t)n_events + 1), cudaMemcpyHostToDevice, st));
     // The staged hit arrays hold hits base .. base+n_sub-1 at positions 0 ..; the kernel indexes them by the (absolute)
     // offsets, so it is handed pointers moved back by `base` -- dereferenced only at base and beyond.
     hough_io io{};
-    io.d_xy = sg->xy - 2 * base; io.d_event_offsets = sg->off; io.n_events = n_events;
+    io.d_xy = sg->xy + 2 * par - 2 * base; io.d_event_offsets = sg->off; io.n_events = n_events;
     io.d_keep_mask = sg->keep - base; io.d_peaks = sg->peaks; io.d_counts = sg->counts;
     io.d_kept_xy = h_kept_xy ? sg->kept_xy - 2 * base : nullptr;
     io.d_kept_idx = h_kept_idx ? sg->kept_idx - base : nullptr;

@@ -106,6 +106,7 @@ struct KParams {
     int theta_wrap;       // column -1 is column n_theta-1 with the rho index mirrored
     int keep_mode;        // 0: (theta, rho) window; 1: distance to the candidate circle
     int circ_cap;         // distance filter: circles staged in the dead accumulator region
+    int stage_mode;       // 0: coalesced float2 loads; 1: one cp.async.bulk per chunk into the hit buffer (north_star (1))
     double keep_tol;      // distance filter tolerance, units of the hit coordinates
 };
 
@@ -139,6 +140,40 @@ __device__ __forceinline__ void vote_add(unsigned saddr, unsigned v) {
 }
 __device__ __forceinline__ void red_shared_or(unsigned saddr, unsigned v) {
     asm volatile("red.shared.or.b32 [%0], %1;" ::"r"(saddr), "r"(v) : "memory");
+}
+#endif
+
+// Bulk-copy staging (EXT, stage_mode 1; north_star subsystem (1), SURVEY.md section 7 "Bulk-copy alignment"): one
+// cp.async.bulk (TMA engine, SASS UBLKCP) per chunk of hits, completion on an mbarrier.  `bar` and `dst` are
+// shared-window addresses, `bytes` a multiple of 16, `src` 16-byte aligned.
+#ifdef HOUGH_HOST_EMU
+inline void mbar_init(unsigned, unsigned) {}
+inline void fence_proxy_async() {}
+inline void mbar_expect_tx(unsigned, unsigned) {}
+inline void bulk_copy_g2s(unsigned dst, const void* src, unsigned bytes, unsigned) {
+    emu::bulk_check(dst, src, bytes);
+    memcpy(emu::shared_ptr(dst), src, bytes);
+    emu::mbar_complete();
+}
+inline bool mbar_try_wait(unsigned, unsigned parity) { return emu::mbar_wait_parity(parity); }
+#else
+__device__ __forceinline__ void mbar_init(unsigned bar, unsigned count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+}
+__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+__device__ __forceinline__ void mbar_expect_tx(unsigned bar, unsigned bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void bulk_copy_g2s(unsigned dst, const void* src, unsigned bytes, unsigned bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(dst), "l"(src), "r"(bytes), "r"(bar) : "memory");
+}
+__device__ __forceinline__ bool mbar_try_wait(unsigned bar, unsigned parity) {
+    unsigned ok;
+    asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+                 : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
+    return ok != 0;
 }
 #endif
 
@@ -276,7 +311,8 @@ __global__ void __launch_bounds__(1024, 1) hough_event_kernel(const __grid_const
 
     unsigned char* acc = smem;                                  // accumulator region
     unsigned* pbm = (unsigned*)(smem + p.pbm_off);              // peak bitmap [cols_per_cta][wpr]
-    float2* hb = (float2*)(smem + p.hb_off);                    // staged (u,v); H4 reuses it as the candidate list
+    float2* const hb0 = (float2*)(smem + p.hb_off);             // staged (u,v); H4 reuses its tail as the candidate list
+    float2* hb = hb0;                                           // (bulk staging shifts it by one hit for odd event starts)
     int* misc = (int*)(smem + p.misc_off);                      // [0..32] scan scratch, [40] peak total, [41] marked count, [42] candidates
     const unsigned acc_s = (unsigned)__cvta_generic_to_shared(acc);
 
@@ -311,6 +347,35 @@ __global__ void __launch_bounds__(1024, 1) hough_event_kernel(const __grid_const
 
     const int zero_vec = (p.region_bytes + p.pbm_bytes) >> 4;   // pbm follows the region; both 16-B multiples
 
+    // EXT, bulk staging: the hit buffer keeps two spare slots (a chunk's source range is aligned down and up by one hit)
+    const bool bulk = EXT && p.stage_mode == 1;
+    const int chunk = bulk ? p.chunk - 2 : p.chunk;
+    const unsigned bar_s = (unsigned)__cvta_generic_to_shared(misc + 52), hb0_s = (unsigned)__cvta_generic_to_shared(hb0);
+    const int total_hits = bulk ? __shfl_sync(0xffffffffu, p.off[p.n_events], 0) : 0;
+    unsigned bar_phase = 0;
+    if (bulk) {
+        if (tid == 0) mbar_init(bar_s, 1u);
+        __syncthreads();
+    }
+    // Issues the copy of chunk [cbeg, cbeg + m) of the event that starts at hit `beg` (thread 0 only).  The 16-byte
+    // aligned source range starts at the even hit index at or below the chunk's first hit and holds an even number of
+    // hits; it may include one hit of a neighbouring event on either side, but never reaches past the batch's last hit:
+    // there the odd last hit is left to a plain load (tail_plain).  Returns the bytes in flight.
+    auto bulk_issue = [&](int beg, int cbeg, int m, int& hshift, bool& tail_plain) -> unsigned {
+        const int g0 = beg + cbeg;
+        hshift = g0 & 1;
+        int cnt = (hshift + m + 1) & ~1;
+        tail_plain = false;
+        if (g0 - hshift + cnt > total_hits) { cnt -= 2; tail_plain = true; }
+        const unsigned bytes = 8u * (unsigned)cnt;
+        if (tid == 0 && cnt > 0 && cnt <= p.chunk) {      // (cnt <= m + 2 <= p.chunk by construction)
+            fence_proxy_async();           // earlier generic-proxy accesses of the buffer are ordered before the async write
+            mbar_expect_tx(bar_s, bytes);
+            bulk_copy_g2s(hb0_s, (const void*)(p.xy + (g0 - hshift)), bytes, bar_s);
+        }
+        return bytes;
+    };
+
     for (int e = cluster_id; e < p.n_events; e += n_clusters) {
         // shfl from lane 0 = "this value is warp-uniform" for ptxas (keeps the event loop in uniform control flow)
         const int beg = __shfl_sync(0xffffffffu, p.off[e], 0);
@@ -320,7 +385,7 @@ __global__ void __launch_bounds__(1024, 1) hough_event_kernel(const __grid_const
             continue;
         }
 
-        const bool single = n <= p.chunk;    // the whole event is staged at once: (u,v) stay in hb until selection
+        const bool single = n <= chunk;      // the whole event is staged at once: (u,v) stay in hb until selection
         int dbg_viol = 0;                    // HOUGH_DEBUG_BOUNDS: first phase whose offset check failed (else unused)
         (void)dbg_viol;
         const unsigned acc_end = (unsigned)(p.n_rho + 1) * (unsigned)p.pitch_b;   // accumulator incl. the trash row
@@ -328,8 +393,13 @@ __global__ void __launch_bounds__(1024, 1) hough_event_kernel(const __grid_const
 
         // the first two hits of this thread are requested before the zeroing stores, which then overlap the latency
         float2 pre0 = make_float2(1.0f, 0.0f), pre1 = pre0;
-        if (tid < n) pre0 = __ldg(&p.xy[beg + tid]);
-        if (tid + nthreads < n) pre1 = __ldg(&p.xy[beg + tid + nthreads]);
+        if (!bulk && tid < n) pre0 = __ldg(&p.xy[beg + tid]);
+        if (!bulk && tid + nthreads < n) pre1 = __ldg(&p.xy[beg + tid + nthreads]);
+        // bulk staging: the first chunk's copy is in flight while the accumulator is zeroed
+        int hshift = 0;
+        bool tail_plain = false;
+        unsigned in_flight = 0;
+        if (bulk && n > 0) in_flight = bulk_issue(beg, 0, min(chunk, n), hshift, tail_plain);
 
         // ---- zero accumulator + peak bitmap
         {
@@ -340,16 +410,27 @@ __global__ void __launch_bounds__(1024, 1) hough_event_kernel(const __grid_const
         }
 
         // ---- H0-H3: stage, transform, vote (chunked)
-        for (int cbeg = 0; cbeg < n; cbeg += p.chunk) {
-            const int m = min(p.chunk, n - cbeg);
+        for (int cbeg = 0; cbeg < n; cbeg += chunk) {
+            const int m = min(chunk, n - cbeg);
             int tame = 1;
+            if (bulk) {
+                if (cbeg > 0) in_flight = bulk_issue(beg, cbeg, m, hshift, tail_plain);   // (the previous chunk ended with a barrier)
+                hb = hb0 + hshift;               // raw hit i of the chunk lands in slot hshift + i: converted in place below
+                if (in_flight) {
+                    bool done = false;
+                    for (int spin = 0; spin < (1 << 24) && !done; ++spin) done = mbar_try_wait(bar_s, bar_phase);   // bounded: never a hang
+                    bar_phase ^= 1u;
+                    if (!done) tail_plain = true, in_flight = 0;      // give up on the copy: every hit comes from a plain load
+                }
+            }
             for (int i = tid; i < m; i += nthreads) {
                 float2 h;
-                if (cbeg == 0 && i == tid) h = pre0;
+                if (bulk) h = (in_flight && !(tail_plain && i == m - 1)) ? hb[i] : __ldg(&p.xy[beg + cbeg + i]);
+                else if (cbeg == 0 && i == tid) h = pre0;
                 else if (cbeg == 0 && i == tid + nthreads) h = pre1;
                 else h = __ldg(&p.xy[beg + cbeg + i]);
                 float2 uv = conformal(h, p.scale);
-                if (HB_CHK(i < p.chunk, HB_STAGE)) hb[i] = uv;
+                if (HB_CHK(hshift + i < p.chunk, HB_STAGE)) hb[i] = uv;
                 const float au = fabsf(uv.x), av = fabsf(uv.y);
                 tame &= (__fadd_rn(au, av) <= p.tame_bound) ? 1 : 0;                        // false for NaN/inf
                 tame &= ((au >= p.ftz_min || au == 0.0f) && (av >= p.ftz_min || av == 0.0f)) ? 1 : 0;
@@ -604,7 +685,7 @@ __global__ void __launch_bounds__(1024, 1) hough_event_kernel(const __grid_const
             // its own thread.  A vector that does not fit the list is handled on the spot, so the list size never
             // decides the result.
             unsigned* vlist = (unsigned*)(hb + (single ? n : 0));
-            const int vcap = 2 * (p.chunk - (single ? n : 0));
+            const int vcap = 2 * (chunk - (single ? n : 0));
             const unsigned thr = (unsigned)p.threshold;
             const int vpr = p.vpr;
             constexpr int CELLS = ACC16 ? 8 : 4;               // cells per uint4
@@ -636,7 +717,7 @@ __global__ void __launch_bounds__(1024, 1) hough_event_kernel(const __grid_const
                 if (!vec_any(w)) return;
                 const int pos = atomicAdd(&misc[42], 1);
                 if (pos < vcap) {
-                    if (HB_CHK((single ? n : 0) * 8 + 4 * pos + 4 <= 8 * p.chunk, HB_H4)) vlist[pos] = (unsigned)v;
+                    if (HB_CHK((hshift + (single ? n : 0)) * 8 + 4 * pos + 4 <= 8 * p.chunk, HB_H4)) vlist[pos] = (unsigned)v;
                     return;
                 }
 #pragma unroll 1
@@ -670,7 +751,7 @@ __global__ void __launch_bounds__(1024, 1) hough_event_kernel(const __grid_const
             __syncthreads();
             const int n_items = min(misc[42], vcap) * CELLS;
             for (int i = tid; i < n_items; i += nthreads)
-                if (HB_CHK((single ? n : 0) * 8 + 4 * (i / CELLS) + 4 <= 8 * p.chunk, HB_H4)) test_cell((int)vlist[i / CELLS], i % CELLS);
+                if (HB_CHK((hshift + (single ? n : 0)) * 8 + 4 * (i / CELLS) + 4 <= 8 * p.chunk, HB_H4)) test_cell((int)vlist[i / CELLS], i % CELLS);
         }
         __syncthreads();
 

@@ -56,15 +56,19 @@ int main(int argc, char** argv) {
     g_acc16 = h[5]; g_cl = h[6]; g_cpl = h[7];
     const int csize = h[8], threads = h[9], smem_bytes = h[10], force_slow = h[11], n_events = h[12], n_total = h[13];
     const int want_kept = h[14], want_accum = h[15], grid_clusters = h[16];
-    const int peak_mode = h[17], rel_permille = h[18], nms_radius = h[19], theta_wrap = h[20], keep_mode = h[21], want_circles = h[22];
-    g_ext = peak_mode != 0 || theta_wrap != 0 || keep_mode != 0;
+    const int peak_mode = h[17], rel_permille = h[18], nms_radius = h[19], theta_wrap = h[20], keep_mode = h[21], want_circles = h[22], stage_mode = h[23];
+    g_ext = peak_mode != 0 || theta_wrap != 0 || keep_mode != 0 || stage_mode != 0;
     std::vector<float> cos_t(n_theta), sin_t(n_theta);
     rd(f, cos_t.data(), n_theta); rd(f, sin_t.data(), n_theta);
     emu::Guarded b_off, b_xy, b_keep, b_peaks, b_counts, b_kxy, b_kidx, b_acc;
     b_off.alloc(4 * (size_t)(n_events + 1));
-    b_xy.alloc(8 * (size_t)n_total + 8);
+    // d_xy is 16-byte aligned (the promise bulk-copy staging relies on); it ends at the guard page when n_total is even,
+    // one hit before it when odd (emu::bulk_check then catches a copy that reads past the batch's last hit)
+    b_xy.alloc(8 * (size_t)n_total + 16);
+    unsigned char* xy_base = b_xy.ptr + ((n_total & 1) ? 8 : 16);
+    emu::bulk_lo = xy_base; emu::bulk_hi = xy_base + 8 * (size_t)n_total;
     rd(f, (int*)b_off.ptr, n_events + 1);
-    rd(f, (float*)(b_xy.ptr + 8), 2 * (size_t)n_total);
+    rd(f, (float*)xy_base, 2 * (size_t)n_total);
     fclose(f);
     const size_t peaks_bytes = 8 * (size_t)n_events * max_peaks, accum_bytes = 4 * (size_t)n_events * n_theta * n_rho;
     b_keep.alloc((size_t)n_total + 1); b_peaks.alloc(peaks_bytes + 8); b_counts.alloc(8 * (size_t)n_events);
@@ -78,7 +82,7 @@ int main(int argc, char** argv) {
 
     kp = hough::KParams();
     // the buffers END at a guard page; an empty buffer still gets a valid pointer (one spare element in front)
-    kp.xy = (const float2*)(b_xy.ptr + 8);
+    kp.xy = (const float2*)xy_base;
     kp.off = (const int*)b_off.ptr;
     kp.n_events = n_events;
     kp.keep = b_keep.ptr + 1;
@@ -99,7 +103,7 @@ int main(int argc, char** argv) {
     kp.colq_off = plan[20]; kp.stash_off = plan[21]; kp.cnt_off = plan[22]; kp.gcnt_off = plan[23];
     kp.rcp_groups = (unsigned)plan[24]; kp.rcp_2s = (unsigned)plan[25]; kp.circ_cap = plan[26];
     kp.peak_mode = peak_mode; kp.rel_permille = rel_permille; kp.nms_radius = nms_radius; kp.theta_wrap = theta_wrap;
-    kp.keep_mode = keep_mode; kp.keep_tol = dbl[0];
+    kp.keep_mode = keep_mode; kp.keep_tol = dbl[0]; kp.stage_mode = stage_mode;
     kp.vpr = kp.pitch_b / 16;
     if (plan[0] != csize || plan[1] != threads || plan[2] != smem_bytes || plan[4] != g_cpl || (plan[3] == 16) != (g_acc16 != 0))
         emu::die("header and plan disagree");

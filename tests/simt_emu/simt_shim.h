@@ -75,6 +75,7 @@ struct Warp {
 };
 
 struct Cta {
+    unsigned mbar_phases = 0;        // completed phases of the CTA's one mbarrier (bulk-copy staging)
     Guarded smem;
     int rank = 0;
     dim3 bidx;
@@ -151,6 +152,29 @@ inline unsigned char* shared_ptr(unsigned saddr) {
 inline unsigned char* dyn_smem() { return cur->cta->smem.ptr; }
 inline int cluster_id() { return g.cluster; }
 inline int n_clusters() { return g.n_clusters_; }
+
+// bulk-copy staging: what a cp.async.bulk must satisfy (16-byte aligned source, destination and size; the source inside
+// the hit array)
+inline const unsigned char* bulk_lo = nullptr;
+inline const unsigned char* bulk_hi = nullptr;
+inline void bulk_check(unsigned dst, const void* src, unsigned bytes) {
+    const unsigned char* s = (const unsigned char*)src;
+    if (((size_t)s & 15) || (bytes & 15) || ((dst - SHARED_WINDOW) & 15)) die("cp.async.bulk: source, destination or size not 16-byte aligned");
+    if (s < bulk_lo || s + bytes > bulk_hi) die("cp.async.bulk: source range leaves the hit array");
+    if ((size_t)(dst - SHARED_WINDOW) + bytes > cur->cta->smem.bytes) die("cp.async.bulk: destination leaves shared memory");
+}
+
+// The CTA's mbarrier: the emulated copy lands at issue time, which completes one phase; a waiter of parity p gets true
+// once the phase of that parity has completed, else it yields (so a thread that runs ahead of the issuing thread really
+// waits, as it does for the asynchronous copy on the device).
+inline void mbar_complete() { ++cur->cta->mbar_phases; }
+inline bool mbar_wait_parity(unsigned parity) {
+    if ((cur->cta->mbar_phases & 1u) != (parity & 1u)) { ++cur->progress; return true; }
+    const unsigned long p0 = cur->progress;
+    yield();
+    cur->progress = p0;
+    return false;
+}
 
 inline float ftz(float x) { return std::fpclassify(x) == FP_SUBNORMAL ? std::copysign(0.0f, x) : x; }
 

@@ -29,11 +29,12 @@ def emu_gpu_ex(_hb, w, xy, off, accum=True, circles=False, cluster_size=0, rho_m
     base = dict(max_peaks=w.max_peaks, acc_dtype=w.acc_dtype, threshold=w.threshold, window=w.window, conformal_scale=1)
     base.update({k: kw.pop(k) for k in list(kw) if k in base})
     opts = {k: kw.pop(k) for k in list(kw) if k in tn.OPTS}
+    emu_only = {k: kw.pop(k) for k in list(kw) if k in tn.GPU_ONLY}
     assert not kw, kw
     rho_max = w.rho_max if rho_max is None else rho_max
     g = simt_emu.run(xy, off, w.n_theta, w.n_rho, rho_max, base["threshold"], base["window"], table, max_peaks=base["max_peaks"],
                      acc_dtype=base["acc_dtype"], accum=accum, conformal_scale=base["conformal_scale"], circles=circles,
-                     cluster_size=cluster_size, debug_bounds=True, **opts)
+                     cluster_size=cluster_size, debug_bounds=True, **opts, **emu_only)
     assert not np.any(g["counts"][:, 0] == -2), "debug-bounds sentinel"
     o, oc = oracle.run_ex(xy, off, w.n_theta, w.n_rho, rho_max, base["threshold"], base["window"], table[0], table[1],
                           max_peaks=base["max_peaks"], conformal_scale=base["conformal_scale"], acc_u16=(base["acc_dtype"] != "u32"),
@@ -92,6 +93,9 @@ NEXT = [
     ("test_n4b_distance_filter", (3, 2, 0, 0.5)),
     ("test_n4b_more_stored_peaks_than_staged_circles", ()),
     ("test_n2_with_theta_wrap_and_on_cluster_grids", ()),
+    ("test_h0_bulk_copy_staging", (0, 16, 0)),
+    ("test_h0_bulk_copy_staging", (1, 8, 4)),
+    ("test_h0_bulk_copy_staging", (5, 2, 0)),
 ]
 
 

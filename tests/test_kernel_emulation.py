@@ -83,9 +83,10 @@ def emu_ex(w, xy, off, accum=True, circles=False, **kw):
     base = dict(max_peaks=w.max_peaks, acc_dtype=w.acc_dtype, threshold=w.threshold, window=w.window, conformal_scale=1)
     base.update({k: kw.pop(k) for k in list(kw) if k in base})
     opts = {k: kw.pop(k) for k in list(kw) if k in ("peak_mode", "rel_permille", "nms_radius", "theta_wrap", "keep_mode", "keep_tol", "b_field")}
+    emu_only = {k: kw.pop(k) for k in list(kw) if k in ("staging", "order")}
     rho_max = kw.pop("rho_max", w.rho_max)
     g = simt_emu.run(xy, off, w.n_theta, w.n_rho, rho_max, base["threshold"], base["window"], table, max_peaks=base["max_peaks"],
-                     acc_dtype=base["acc_dtype"], accum=accum, conformal_scale=base["conformal_scale"], circles=circles, **opts, **kw)
+                     acc_dtype=base["acc_dtype"], accum=accum, conformal_scale=base["conformal_scale"], circles=circles, **opts, **emu_only, **kw)
     o, oc = oracle.run_ex(xy, off, w.n_theta, w.n_rho, rho_max, base["threshold"], base["window"], table[0], table[1],
                           max_peaks=base["max_peaks"], conformal_scale=base["conformal_scale"], acc_u16=(base["acc_dtype"] != "u32"),
                           want_accum=accum, n_threads=4, want_circles=circles, **opts)
@@ -169,3 +170,34 @@ def test_results_do_not_depend_on_the_order_in_which_threads_reach_their_barrier
     xy3, off3, _ = si.generate(w3, 4)
     big = np.ascontiguousarray(xy3[:off3[4]])          # ~11000 hits as one event: several staging chunks, several selection blocks
     emu_both(w3, big, np.array([0, len(big)], dtype=np.int32), threshold=45, cluster_size=2, order=order)
+
+
+# ---------------------------------------------------------------- bulk-copy staging (HOUGH_OPT_STAGING = 1) under the emulator
+@pytest.mark.parametrize("cfg,n_ev,cluster", [(0, 5, 0), (1, 3, 0), (0, 4, 2), (3, 2, 0)])
+def test_bulk_copy_staging_under_the_emulator(cfg, n_ev, cluster):
+    # events start at odd and even hit indices; the emulator checks every copy: 16-byte aligned source, destination and
+    # size, source inside the hit array (the batch's odd last hit must come from a plain load)
+    w = si.config(cfg)
+    xy, off, _ = si.generate(w, n_ev)
+    emu_ex(w, xy, off, staging=1, cluster_size=cluster, debug_bounds=True)
+    # without the batch's first hit every later event starts at the other parity, and the batch ends on the other parity
+    off2 = np.concatenate([[0], off[1:] - 1]).astype(np.int32)
+    emu_ex(w, xy[1:], off2, staging=1, cluster_size=cluster, debug_bounds=True)
+    assert {int(o) & 1 for o in off[1:-1]} | {int(o) & 1 for o in off2[1:-1]} == {0, 1} and (len(xy) - 1) % 2 != len(xy) % 2
+
+
+def test_bulk_copy_staging_edge_cases_under_the_emulator():
+    w = si.config(0)
+    xy, off, _ = si.generate(w, 3)
+    # empty events, one-hit and two-hit events, the last event a single (odd) hit
+    xy1 = np.concatenate([xy[:off[1]], np.array([[300, 0], [0, 450], [200, 200], [-700, 100]], dtype=np.float32)])
+    off1 = np.array([0, 0, off[1], off[1] + 1, off[1] + 3, off[1] + 3, off[1] + 4], dtype=np.int32)
+    emu_ex(w, xy1, off1, staging=1, threshold=1, max_peaks=512, debug_bounds=True)
+    # an event larger than the staging chunk: several copies per event, every chunk with its own alignment shift
+    w3 = si.config(3)
+    xy3, off3, _ = si.generate(w3, 4)
+    big = np.ascontiguousarray(xy3[1:off3[4]])
+    emu_ex(w3, big, np.array([0, 5, len(big)], dtype=np.int32), staging=1, threshold=45, debug_bounds=True)
+    emu_ex(w3, big, np.array([0, 5, len(big)], dtype=np.int32), staging=1, threshold=45, cluster_size=2, acc_dtype="u16", order="shuffle:3")
+    # together with the other options of the extended instantiation
+    emu_ex(w, xy, off, staging=1, peak_mode=1, theta_wrap=True, keep_mode=1, keep_tol=5.0, circles=True)

@@ -11,6 +11,7 @@ from tests.test_parity_gpu import compare
 pytestmark = pytest.mark.gpu
 
 OPTS = ("peak_mode", "rel_permille", "nms_radius", "theta_wrap", "keep_mode", "keep_tol", "b_field")
+GPU_ONLY = ("staging",)          # same results by definition: the oracle has no such option
 
 
 @pytest.fixture(scope="module")
@@ -28,10 +29,11 @@ def gpu_ex(hb, w, xy, off, accum=True, circles=False, cluster_size=0, rho_max=No
     base = dict(max_peaks=w.max_peaks, acc_dtype=w.acc_dtype, threshold=w.threshold, window=w.window, conformal_scale=1)
     base.update({k: kw.pop(k) for k in list(kw) if k in base})
     opts = {k: kw.pop(k) for k in list(kw) if k in OPTS}
+    gpu_only = {k: kw.pop(k) for k in list(kw) if k in GPU_ONLY}
     assert not kw, kw
     rho_max = w.rho_max if rho_max is None else rho_max
     h = hb.Hough(w.n_theta, w.n_rho, rho_max, base["threshold"], base["window"], max_peaks=base["max_peaks"], acc_dtype=base["acc_dtype"],
-                 conformal_scale=base["conformal_scale"], cluster_size=cluster_size, trig_table=table, **opts)
+                 conformal_scale=base["conformal_scale"], cluster_size=cluster_size, trig_table=table, **opts, **gpu_only)
     try:
         d_xy = torch.from_numpy(np.ascontiguousarray(xy, dtype=np.float32).reshape(-1, 2)).cuda()
         d_off = torch.from_numpy(np.ascontiguousarray(off, dtype=np.int32)).cuda()
@@ -228,4 +230,32 @@ def test_n4c_host_sub_batches_on_several_streams_overlap_safely(hb):
         hb.hough_run_host(h.ctx, h_xy, h_off[e0:], 20, keep, peaks[e0:], counts[e0:], None, None, stream=many[b])
     torch.cuda.synchronize()
     assert np.array_equal(counts.numpy(), o.counts) and np.array_equal(keep.numpy(), o.keep)
+    h.close()
+
+
+# ---------------------------------------------------------------- H0 variant: bulk-copy (TMA engine) staging.  Kept last in the
+# file: it is the one path whose PTX (cp.async.bulk + mbarrier) has no CPU restatement beyond a memcpy.  The wait on the
+# mbarrier is bounded in the kernel, so a mistake shows up as a mismatch, never as a hang.
+@pytest.mark.parametrize("cfg,n_ev,cluster", [(0, 16, 0), (1, 100, 0), (3, 6, 0), (5, 12, 0), (1, 30, 4)])
+def test_h0_bulk_copy_staging(hb, cfg, n_ev, cluster):
+    w = si.config(cfg)
+    xy, off, _ = si.generate(w, n_ev)
+    gpu_ex(hb, w, xy, off, staging=1, cluster_size=cluster)
+    # without the batch's first hit every event starts at the other parity and the batch ends on the other parity
+    gpu_ex(hb, w, np.ascontiguousarray(xy[1:]), np.concatenate([[0], off[1:] - 1]).astype(np.int32), staging=1, cluster_size=cluster, accum=False)
+
+
+def test_h0_bulk_copy_staging_chunked_events_and_alignment_check(hb):
+    import torch
+    w3 = si.config(3)
+    xy3, off3, _ = si.generate(w3, 6)
+    big = np.ascontiguousarray(xy3[1:off3[6]])                       # ~17000 hits in one event: several copies, each with its own shift
+    gpu_ex(hb, w3, big, np.array([0, 5, len(big)], dtype=np.int32), staging=1, threshold=60)
+    w = si.config(0)
+    xy, off, _ = si.generate(w, 4)
+    h = hb.Hough(w.n_theta, w.n_rho, w.rho_max, w.threshold, w.window, staging=1)
+    d = torch.from_numpy(np.concatenate([xy[:1], xy])).cuda()      # a view that starts 8 bytes into the allocation
+    out = h.alloc_outputs(len(xy), 4)
+    with pytest.raises(hb.HoughError, match="16-byte"):
+        hb.hough_run(h.ctx, d[1:], torch.from_numpy(off).cuda(), 4, out["keep"], out["peaks"], out["counts"])
     h.close()

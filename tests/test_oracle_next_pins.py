@@ -217,7 +217,7 @@ def nms_numpy(A, thr, permille, radius, wrap=False):
 def test_n2_against_numpy_restatement_and_invariants(wrap):
     rng = np.random.default_rng(4)
     cases = [rng.poisson(2.0, size=(rng.integers(2, 24), rng.integers(2, 24))).astype(np.uint32) for _ in range(25)]
-    w = si.config(1)
+    w = si.config(0)
     xy, off, _ = si.generate(w, 2)
     t = si.trig_table(w.n_theta)
     cases += list(oracle.run(xy, off, w.n_theta, w.n_rho, w.rho_max, w.threshold, w.window, t[0], t[1], want_accum=True).accum)

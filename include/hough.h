@@ -95,11 +95,18 @@ typedef enum hough_option {
     HOUGH_OPT_KEEP_MODE = 11,       /* 0 = (theta, rho) window around the stored peaks (default); 1 = original-space road
                                        | ||hit - centre|| - r_c | < HOUGH_OPTF_KEEP_TOL around their candidate circles
                                        ("inversely mapped back to the original space ... data filtering") */
-    HOUGH_OPT_STAGING = 12          /* how an event's hits reach shared memory (H0; PAPER.md:86 names non-coalesced access
+    HOUGH_OPT_STAGING = 12,         /* how an event's hits reach shared memory (H0; PAPER.md:86 names non-coalesced access
                                        as a hazard): 0 = coalesced float2 loads issued ahead of the zeroing stores (default);
                                        1 = one cp.async.bulk (TMA engine) per chunk, completion on an mbarrier, the 16-byte
                                        aligned source range found by aligning down and up by one hit; needs d_xy 16-byte
                                        aligned.  Same results; never yet timed */
+    HOUGH_OPT_SCHEDULER = 13        /* how events reach the SMs (events "assigned to different thread blocks"):
+                                       0 = one CTA (cluster) per event, dealt by the hardware block scheduler (default);
+                                       1 = the same launch, but a resident CTA cancels the launch of a not-yet-started CTA
+                                       (Blackwell cluster launch control) and takes over its event, so the per-CTA set-up
+                                       runs once per resident CTA, and the next event's hits are prefetched into L2 under
+                                       the current event's peak finding and selection; one-CTA-per-event grids only (a
+                                       clustered grid ignores it); needs d_xy 16-byte aligned.  Same results; never yet timed */
 } hough_option;
 
 typedef enum hough_option_f64 {

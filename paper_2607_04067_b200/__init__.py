@@ -29,6 +29,7 @@ HOUGH_OPT_NMS_RADIUS = 9
 HOUGH_OPT_THETA_WRAP = 10
 HOUGH_OPT_KEEP_MODE = 11
 HOUGH_OPT_STAGING = 12
+HOUGH_OPT_SCHEDULER = 13
 HOUGH_OPTF_KEEP_TOL = 1
 HOUGH_OPTF_B_FIELD_TESLA = 2
 HOUGH_ACC_AUTO, HOUGH_ACC_U16, HOUGH_ACC_U32 = 0, 1, 2
@@ -344,7 +345,7 @@ class Hough:
 
     def __init__(self, n_theta, n_rho, rho_max, threshold, window, max_peaks=64, acc_dtype="u16",
                  conformal_scale=1, cluster_size=0, ctas_per_sm=0, trig_table=None, peak_mode=0, rel_permille=500,
-                 nms_radius=1, theta_wrap=False, keep_mode=0, keep_tol=0.0, b_field=1.0, staging=0):
+                 nms_radius=1, theta_wrap=False, keep_mode=0, keep_tol=0.0, b_field=1.0, staging=0, scheduler=0):
         self.n_theta, self.n_rho, self.max_peaks = n_theta, n_rho, max_peaks
         self.ctx = hough_create(n_theta, n_rho, float(rho_max), threshold, window)
         try:
@@ -371,6 +372,8 @@ class Hough:
                 hough_set_option_f64(self.ctx, HOUGH_OPTF_B_FIELD_TESLA, b_field)
             if staging:
                 hough_set_option(self.ctx, HOUGH_OPT_STAGING, staging)
+            if scheduler:
+                hough_set_option(self.ctx, HOUGH_OPT_SCHEDULER, scheduler)
         except Exception:
             self.close()
             raise

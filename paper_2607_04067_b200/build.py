@@ -9,8 +9,8 @@
 
 The kernels use __fmul_rn/__fadd_rn/__fadd_rd and -fmad=false so that no multiply-add is ever contracted (DESIGN.md
 S2); as a belt-and-braces check the product's SASS must contain no packed FFMA2 and must contain the floor-add
-(FADD.RM), the clamp (VIMNMX) and the vote (ATOMS.POPC.INC); the bulk-copy staging option must show up as UBLKCP, and only
-in the extended instantiations."""
+(FADD.RM), the clamp (VIMNMX) and the vote (ATOMS.POPC.INC); the bulk-copy staging option must show up as UBLKCP, the work-stealing
+scheduler as UGETNEXTWORKID (cluster launch control) and UBLKPF (L2 prefetch), and only in the extended instantiations."""
 import os
 import re
 import subprocess
@@ -57,13 +57,13 @@ def check_sass(lib: str = LIB) -> None:
     sass = _sass(lib)
     if "FFMA2" in sass:
         raise RuntimeError("ptxas contracted a packed fp32 multiply-add (FFMA2 found): bit-exactness is lost")
-    for needle in ("FADD.RM", "ATOMS.POPC.INC", "VIMNMX", "UBLKCP"):
+    for needle in ("FADD.RM", "ATOMS.POPC.INC", "VIMNMX", "UBLKCP", "UGETNEXTWORKID", "UBLKPF"):
         if needle not in sass:
             raise RuntimeError("expected %s in the SASS of %s" % (needle, lib))
     # the default instantiations (EXT = false, last template argument Lb0E) carry none of the optional paths:
-    # no bulk copy / mbarrier, no fp64 arithmetic of the distance filter
+    # no bulk copy / mbarrier / launch control, no fp64 arithmetic of the distance filter
     for m in re.finditer(r"Function : (\S*hough_event_kernelI\S*ELb0EEE\S*)\n(.*?)(?=\n\s*Function : |\Z)", sass, flags=re.S):
-        for needle in ("UBLKCP", "SYNCS", "DADD", "DMUL", "DFMA"):
+        for needle in ("UBLKCP", "UBLKPF", "UGETNEXTWORKID", "SYNCS", "DADD", "DMUL", "DFMA"):
             if needle in m.group(2):
                 raise RuntimeError("%s found in the default instantiation %s" % (needle, m.group(1)))
 

@@ -107,6 +107,7 @@ struct KParams {
     int keep_mode;        // 0: (theta, rho) window; 1: distance to the candidate circle
     int circ_cap;         // distance filter: circles staged in the dead accumulator region
     int stage_mode;       // 0: coalesced float2 loads; 1: one cp.async.bulk per chunk into the hit buffer (north_star (1))
+    int sched_mode;       // 0: one CTA per event; 1: a resident CTA steals not-yet-launched CTAs' events (cluster launch control)
     double keep_tol;      // distance filter tolerance, units of the hit coordinates
 };
 
@@ -150,12 +151,24 @@ __device__ __forceinline__ void red_shared_or(unsigned saddr, unsigned v) {
 inline void mbar_init(unsigned, unsigned) {}
 inline void fence_proxy_async() {}
 inline void mbar_expect_tx(unsigned, unsigned) {}
-inline void bulk_copy_g2s(unsigned dst, const void* src, unsigned bytes, unsigned) {
+inline void bulk_copy_g2s(unsigned dst, const void* src, unsigned bytes, unsigned bar) {
     emu::bulk_check(dst, src, bytes);
     memcpy(emu::shared_ptr(dst), src, bytes);
-    emu::mbar_complete();
+    emu::mbar_complete(bar);
 }
-inline bool mbar_try_wait(unsigned, unsigned parity) { return emu::mbar_wait_parity(parity); }
+inline bool mbar_try_wait(unsigned bar, unsigned parity) { return emu::mbar_wait_parity(bar, parity); }
+inline void prefetch_l2_bulk(const void*, unsigned) {}
+// cluster launch control: the emulator hands out the not-yet-launched CTAs of the grid (emu::clc_steal)
+inline void clc_try_cancel(unsigned resp, unsigned bar) {
+    int* r = (int*)emu::shared_ptr(resp);
+    const int id = emu::clc_steal();
+    r[0] = id; r[1] = 0; r[2] = 0; r[3] = id >= 0 ? 1 : 0;
+    emu::mbar_complete(bar);
+}
+inline int clc_query(unsigned resp) {        // the stolen CTA's blockIdx.x, or -1 when nothing was left to steal
+    const int* r = (const int*)emu::shared_ptr(resp);
+    return r[3] ? r[0] : -1;
+}
 #else
 __device__ __forceinline__ void mbar_init(unsigned bar, unsigned count) {
     asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
@@ -168,6 +181,25 @@ __device__ __forceinline__ void mbar_expect_tx(unsigned bar, unsigned bytes) {
 __device__ __forceinline__ void bulk_copy_g2s(unsigned dst, const void* src, unsigned bytes, unsigned bar) {
     asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
                  ::"r"(dst), "l"(src), "r"(bytes), "r"(bar) : "memory");
+}
+// L2 prefetch of a 16-byte aligned global range (a hint: no destination, no completion to wait for)
+__device__ __forceinline__ void prefetch_l2_bulk(const void* src, unsigned bytes) {
+    asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(src), "r"(bytes) : "memory");
+}
+// Blackwell cluster launch control (PTX ISA 8.6, sm_100): ask the hardware to cancel the launch of a CTA of this grid
+// that has not started yet; the 16-byte answer lands in shared memory and completes 16 bytes on the mbarrier.
+__device__ __forceinline__ void clc_try_cancel(unsigned resp, unsigned bar) {
+    asm volatile("clusterlaunchcontrol.try_cancel.async.shared::cta.mbarrier::complete_tx::bytes.b128 [%0], [%1];"
+                 ::"r"(resp), "r"(bar) : "memory");
+}
+// Decodes the answer: the cancelled CTA's blockIdx.x (this CTA now owns its work), or -1 when no CTA was left.
+__device__ __forceinline__ int clc_query(unsigned resp) {
+    unsigned ok, x;
+    asm volatile("{\n\t.reg .pred p;\n\t.reg .b128 r;\n\tld.shared.b128 r, [%2];\n\t"
+                 "clusterlaunchcontrol.query_cancel.is_canceled.pred.b128 p, r;\n\tselp.u32 %0, 1, 0, p;\n\tmov.u32 %1, 0;\n\t"
+                 "@p clusterlaunchcontrol.query_cancel.get_first_ctaid::x.b32.b128 %1, r;\n\t}"
+                 : "=r"(ok), "=r"(x) : "r"(resp) : "memory");
+    return ok ? (int)x : -1;
 }
 __device__ __forceinline__ bool mbar_try_wait(unsigned bar, unsigned parity) {
     unsigned ok;
@@ -351,7 +383,7 @@ __global__ void __launch_bounds__(1024, 1) hough_event_kernel(const __grid_const
     const bool bulk = EXT && p.stage_mode == 1;
     const int chunk = bulk ? p.chunk - 2 : p.chunk;
     const unsigned bar_s = (unsigned)__cvta_generic_to_shared(misc + 52), hb0_s = (unsigned)__cvta_generic_to_shared(hb0);
-    const int total_hits = bulk ? __shfl_sync(0xffffffffu, p.off[p.n_events], 0) : 0;
+    const int total_hits = (bulk || (EXT && !CL && p.sched_mode == 1)) ? __shfl_sync(0xffffffffu, p.off[p.n_events], 0) : 0;
     unsigned bar_phase = 0;
     if (bulk) {
         if (tid == 0) mbar_init(bar_s, 1u);
@@ -376,7 +408,40 @@ __global__ void __launch_bounds__(1024, 1) hough_event_kernel(const __grid_const
         return bytes;
     };
 
-    for (int e = cluster_id; e < p.n_events; e += n_clusters) {
+    // EXT, scheduler mode 1 (one CTA per event only): persistent CTAs with hardware work stealing.  The launch is the same
+    // one-CTA-per-event grid; a resident CTA asks, at the start of every event, to cancel the launch of a CTA that has not
+    // started yet (cluster launch control) and, when its own event is done, takes over the cancelled CTA's event: the
+    // per-CTA prologue above (table loads, lane constants) then runs once per resident CTA, the block scheduler still
+    // balances the events, and no scratch memory or counter is needed (the handle stays re-entrant).  The answer arrives
+    // long before it is needed; when it names a next event, that event's hits are prefetched into L2 while this event's
+    // H4-H7 run.  A failed request (nothing left to launch) ends the loop: no request may follow a failed one.
+    const bool steal = EXT && !CL && p.sched_mode == 1;
+    const unsigned clc_bar_s = (unsigned)__cvta_generic_to_shared(misc + 56), clc_resp_s = (unsigned)__cvta_generic_to_shared(misc + 60);
+    unsigned clc_phase = 0;
+    if (steal) {
+        if (tid == 0) mbar_init(clc_bar_s, 1u);
+        __syncthreads();
+    }
+    auto next_event = [&](int e) -> int {
+        if (!steal) return e + n_clusters;
+        __syncthreads();                           // every thread is done with event e (and with the previous answer)
+        if (tid == 0) {
+            bool done = false;
+            for (int spin = 0; spin < (1 << 24) && !done; ++spin) done = mbar_try_wait(clc_bar_s, clc_phase);   // bounded: never a hang
+            misc[54] = done ? clc_query(clc_resp_s) : -1;
+        }
+        clc_phase ^= 1u;
+        __syncthreads();
+        const int nxt = misc[54];
+        return nxt >= 0 ? nxt : p.n_events;        // p.n_events ends the loop
+    };
+
+    for (int e = cluster_id; e < p.n_events; e = next_event(e)) {
+        if (steal && tid == 0) {                   // this event's request: answered while the event is processed
+            fence_proxy_async();                   // the previous answer was read through the generic proxy
+            mbar_expect_tx(clc_bar_s, 16u);
+            clc_try_cancel(clc_resp_s, clc_bar_s);
+        }
         // shfl from lane 0 = "this value is warp-uniform" for ptxas (keeps the event loop in uniform control flow)
         const int beg = __shfl_sync(0xffffffffu, p.off[e], 0);
         const int n = __shfl_sync(0xffffffffu, p.off[e + 1], 0) - beg;
@@ -487,6 +552,16 @@ __global__ void __launch_bounds__(1024, 1) hough_event_kernel(const __grid_const
         }
         if (n == 0) __syncthreads();         // no staging barrier ran: order the zeroing before the scan
         if (CL) cg::this_cluster().sync();   // (A) every CTA's columns are complete
+
+        // scheduler mode 1: if the answer to this event's request is already there, pull the next event's hits into L2
+        // now, under this event's H4-H7 (a hint only; the 16-byte aligned range never reaches past the batch's last hit)
+        if (steal && tid == 0 && mbar_try_wait(clc_bar_s, clc_phase)) {
+            const int nxt = clc_query(clc_resp_s);
+            if (nxt >= 0 && nxt < p.n_events) {
+                const int b0 = p.off[nxt] & ~1, b1 = min((p.off[nxt + 1] + 1) & ~1, total_hits & ~1);
+                if (b1 > b0) prefetch_l2_bulk((const void*)(p.xy + b0), 8u * (unsigned)(b1 - b0));
+            }
+        }
 
 #ifdef HOUGH_DIAG
         if (p.diag == 3) { __syncthreads(); continue; }

@@ -75,7 +75,9 @@ struct Warp {
 };
 
 struct Cta {
-    unsigned mbar_phases = 0;        // completed phases of the CTA's one mbarrier (bulk-copy staging)
+    unsigned mbar_phases[2] = {0, 0};   // completed phases of the CTA's mbarriers (bulk-copy staging, launch control)
+    unsigned mbar_addr[2] = {0, 0};
+    int steals_left = 0;             // launch control: how many more events this CTA may take over (emu::clc_steal)
     Guarded smem;
     int rank = 0;
     dim3 bidx;
@@ -167,13 +169,29 @@ inline void bulk_check(unsigned dst, const void* src, unsigned bytes) {
 // The CTA's mbarrier: the emulated copy lands at issue time, which completes one phase; a waiter of parity p gets true
 // once the phase of that parity has completed, else it yields (so a thread that runs ahead of the issuing thread really
 // waits, as it does for the asynchronous copy on the device).
-inline void mbar_complete() { ++cur->cta->mbar_phases; }
-inline bool mbar_wait_parity(unsigned parity) {
-    if ((cur->cta->mbar_phases & 1u) != (parity & 1u)) { ++cur->progress; return true; }
-    const unsigned long p0 = cur->progress;
+inline unsigned& mbar_slot(unsigned bar) {
+    Cta* c = cur->cta;
+    for (int i = 0; i < 2; ++i) {
+        if (c->mbar_addr[i] == bar) return c->mbar_phases[i];
+        if (c->mbar_addr[i] == 0) { c->mbar_addr[i] = bar; return c->mbar_phases[i]; }
+    }
+    die("more than two mbarriers in one CTA");
+}
+inline void mbar_complete(unsigned bar) { ++mbar_slot(bar); }
+inline bool mbar_wait_parity(unsigned bar, unsigned parity) {
+    if ((mbar_slot(bar) & 1u) != (parity & 1u)) { ++cur->progress; return true; }
     yield();
-    cur->progress = p0;
     return false;
+}
+// Cluster launch control: the CTAs of the grid that have not started yet are cluster ids next_unlaunched .. n-1 (the
+// emulator runs one CTA after the other).  A request hands out the next of them -- the hardware then never launches it
+// -- unless this CTA has used up its share (HOUGH_EMU_STEALS, default unlimited; a small number mixes stolen and
+// regularly launched CTAs) or none is left; -1 = the request failed.
+inline int next_unlaunched = 0;
+inline int clc_steal() {
+    if (cur->cta->steals_left == 0 || next_unlaunched >= g.n_clusters_) return -1;
+    if (cur->cta->steals_left > 0) --cur->cta->steals_left;
+    return next_unlaunched++;
 }
 
 inline float ftz(float x) { return std::fpclassify(x) == FP_SUBNORMAL ? std::copysign(0.0f, x) : x; }
@@ -201,6 +219,7 @@ inline void run_cluster(int cluster, int n_clusters, int csize, int threads, siz
         c.bidx.x = (unsigned)(cluster * csize + r);
         c.bar.expected = threads;
         c.warps.assign((size_t)threads / 32, Warp());
+        c.steals_left = getenv("HOUGH_EMU_STEALS") ? atoi(getenv("HOUGH_EMU_STEALS")) : -1;
         for (int t = 0; t < threads; ++t) {
             Fiber& f = fibers[(size_t)r * threads + t];
             f.stack.resize(32 * 1024);

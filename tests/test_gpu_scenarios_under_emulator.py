@@ -96,6 +96,8 @@ NEXT = [
     ("test_h0_bulk_copy_staging", (0, 16, 0)),
     ("test_h0_bulk_copy_staging", (1, 8, 4)),
     ("test_h0_bulk_copy_staging", (5, 2, 0)),
+    ("test_work_stealing_scheduler", (0, 16, 0)),
+    ("test_work_stealing_scheduler", (1, 12, 1)),
 ]
 
 

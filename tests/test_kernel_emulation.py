@@ -83,7 +83,7 @@ def emu_ex(w, xy, off, accum=True, circles=False, **kw):
     base = dict(max_peaks=w.max_peaks, acc_dtype=w.acc_dtype, threshold=w.threshold, window=w.window, conformal_scale=1)
     base.update({k: kw.pop(k) for k in list(kw) if k in base})
     opts = {k: kw.pop(k) for k in list(kw) if k in ("peak_mode", "rel_permille", "nms_radius", "theta_wrap", "keep_mode", "keep_tol", "b_field")}
-    emu_only = {k: kw.pop(k) for k in list(kw) if k in ("staging", "order")}
+    emu_only = {k: kw.pop(k) for k in list(kw) if k in ("staging", "order", "scheduler", "steals")}
     rho_max = kw.pop("rho_max", w.rho_max)
     g = simt_emu.run(xy, off, w.n_theta, w.n_rho, rho_max, base["threshold"], base["window"], table, max_peaks=base["max_peaks"],
                      acc_dtype=base["acc_dtype"], accum=accum, conformal_scale=base["conformal_scale"], circles=circles, **opts, **emu_only, **kw)
@@ -201,3 +201,23 @@ def test_bulk_copy_staging_edge_cases_under_the_emulator():
     emu_ex(w3, big, np.array([0, 5, len(big)], dtype=np.int32), staging=1, threshold=45, cluster_size=2, acc_dtype="u16", order="shuffle:3")
     # together with the other options of the extended instantiation
     emu_ex(w, xy, off, staging=1, peak_mode=1, theta_wrap=True, keep_mode=1, keep_tol=5.0, circles=True)
+
+
+# ---------------------------------------------------------------- work-stealing scheduler (HOUGH_OPT_SCHEDULER = 1) under the emulator
+@pytest.mark.parametrize("steals", [None, 0, 1, 3])
+def test_work_stealing_scheduler_under_the_emulator(steals):
+    # the emulator runs one CTA after the other and hands a running CTA's cancellation requests the not-yet-launched
+    # CTAs: without a limit the first CTA takes over every event; steals = 0 makes every request fail (one event per CTA,
+    # as without the option); small limits mix stolen and regularly launched CTAs.  Every event must come out exactly
+    # once and bit-identical, empty / refused / chunked events included.
+    w = si.config(0)
+    xy, off, _ = si.generate(w, 7)
+    off2 = np.concatenate([[0, 0], off[1:4], [off[3]], off[4:]]).astype(np.int32)      # two empty events in between
+    emu_ex(w, xy, off2, scheduler=1, steals=steals, debug_bounds=True)
+    emu_ex(w, xy, off2, scheduler=1, staging=1, steals=steals, circles=True, peak_mode=1, order="shuffle:5")
+    w3 = si.config(3)
+    xy3, off3, _ = si.generate(w3, 3)
+    big = np.ascontiguousarray(xy3[:off3[3]])
+    emu_ex(w3, big, np.array([0, 7, len(big) - 3, len(big)], dtype=np.int32), scheduler=1, steals=steals, threshold=45)
+    # clustered grids ignore the option
+    emu_ex(w, xy, off, scheduler=1, steals=steals, cluster_size=2)

@@ -11,7 +11,7 @@ from tests.test_parity_gpu import compare
 pytestmark = pytest.mark.gpu
 
 OPTS = ("peak_mode", "rel_permille", "nms_radius", "theta_wrap", "keep_mode", "keep_tol", "b_field")
-GPU_ONLY = ("staging",)          # same results by definition: the oracle has no such option
+GPU_ONLY = ("staging", "scheduler")          # same results by definition: the oracle has no such options
 
 
 @pytest.fixture(scope="module")
@@ -258,4 +258,40 @@ def test_h0_bulk_copy_staging_chunked_events_and_alignment_check(hb):
     out = h.alloc_outputs(len(xy), 4)
     with pytest.raises(hb.HoughError, match="16-byte"):
         hb.hough_run(h.ctx, d[1:], torch.from_numpy(off).cuda(), 4, out["keep"], out["peaks"], out["counts"])
+    h.close()
+
+
+# ---------------------------------------------------------------- scheduler variant: persistent CTAs that steal not-yet-launched
+# CTAs' events (cluster launch control) and prefetch the next event's hits into L2.  Bounded waits: a mistake is a mismatch.
+@pytest.mark.parametrize("cfg,n_ev,staging", [(0, 16, 0), (1, 1000, 0), (1, 400, 1), (2, 300, 0), (3, 200, 1)])
+def test_work_stealing_scheduler(hb, cfg, n_ev, staging):
+    # more events than resident CTA slots (296 for the 180 x 256 u16 grid), so that requests succeed AND fail
+    w = si.config(cfg)
+    xy, off, _ = si.generate(w, n_ev)
+    gpu_ex(hb, w, xy, off, scheduler=1, staging=staging, accum=False)
+
+
+def test_work_stealing_scheduler_with_empty_refused_and_chunked_events_and_on_streams(hb):
+    import torch
+    w = si.config(1)
+    xy, off, _ = si.generate(w, 600)
+    off2 = np.concatenate([[0, 0], off[1:300], [off[299]], off[300:]]).astype(np.int32)        # empty events in between
+    gpu_ex(hb, w, xy, off2, scheduler=1, accum=False)
+    w3 = si.config(3)
+    xy3, off3, _ = si.generate(w3, 400)
+    cut = int(off3[6])
+    off_big = np.concatenate([[0, cut], off3[7:]]).astype(np.int32)                            # the first event has ~17000 hits
+    gpu_ex(hb, w3, xy3, off_big, scheduler=1, threshold=60, accum=False)
+    # the same handle on three streams at once (no scratch, no counter: the requests of different launches never mix)
+    table = si.trig_table(w.n_theta)
+    o = oracle.run(xy, off, w.n_theta, w.n_rho, w.rho_max, w.threshold, w.window, table[0], table[1], max_peaks=w.max_peaks, n_threads=8)
+    h = hb.Hough(w.n_theta, w.n_rho, w.rho_max, w.threshold, w.window, trig_table=table, scheduler=1)
+    d_xy, d_off = torch.from_numpy(xy).cuda(), torch.from_numpy(off).cuda()
+    outs, streams = [], [torch.cuda.Stream() for _ in range(3)]
+    torch.cuda.synchronize()
+    for s in streams:
+        outs.append(h.run(d_xy, d_off, stream=s, kept=False))
+    torch.cuda.synchronize()
+    for out in outs:
+        assert np.array_equal(out["counts"].cpu().numpy(), o.counts) and np.array_equal(out["keep"].cpu().numpy(), o.keep)
     h.close()

@@ -451,7 +451,7 @@ def test_measurement_aids_run(hb):
 # round-1 suite so that `pytest -x` reaches those first)
 def test_forced_cluster_of_eight_matches_oracle(hb):
     w = si.config(1)
-    xy, off, _ = si.generate(w, 40)
+    xy, off, _ = si.generate(w, 12)
     g, _ = run_both(hb, w, xy, off, cluster_size=8)
     assert g["info"]["CLUSTER_SIZE"] == 8
 
@@ -459,7 +459,7 @@ def test_forced_cluster_of_eight_matches_oracle(hb):
 def test_cluster_grid_360x512_u32_plans_eight_ctas(hb):
     # 720 KB of u32 cells: 90 columns per CTA pad to 128 (262 KB, too much), so the planner takes 8 CTAs of 45 columns
     w = si.config(5)
-    xy, off, _ = si.generate(w, 16)
+    xy, off, _ = si.generate(w, 5)
     g, _ = run_both(hb, w, xy, off, acc_dtype="u32")
     assert g["info"]["CLUSTER_SIZE"] == 8 and g["info"]["ACC_BITS"] == 32
 

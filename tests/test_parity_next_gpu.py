@@ -133,9 +133,10 @@ def test_n2_with_theta_wrap_and_on_cluster_grids(hb):
     gpu_ex(hb, w0, xy, off, peak_mode=1, rel_permille=300, nms_radius=2, theta_wrap=True, threshold=12)
     # theta columns split over a cluster: one cluster barrier per extracted peak, the same decision in every CTA
     w5 = si.config(5)
-    xy, off, _ = si.generate(w5, 3)
+    xy, off, _ = si.generate(w5, 2)
     gpu_ex(hb, w5, xy, off, peak_mode=1, rel_permille=400, nms_radius=2)
     xy, off = seam_events(w0, 4)
+    xy, off = seam_events(w0, 2)
     for cluster in (2, 8):
         gpu_ex(hb, w0, xy, off, peak_mode=1, rel_permille=300, nms_radius=3, theta_wrap=True, threshold=12, cluster_size=cluster, circles=True)
 

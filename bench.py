@@ -212,7 +212,7 @@ class Workbench:
         self.hb, self.torch, self.dev = hb, torch, dev
         self.w = w = si.config(cfg)
         self.n_events = n_events
-        self.xy, self.off, _ = si.generate(w, n_events, first_event=first_event)
+        self.xy, self.off, self.truth = si.generate(w, n_events, first_event=first_event)
         self.n_total = len(self.xy)
         self.table = si.trig_table(w.n_theta)
         self.h = hb.Hough(w.n_theta, w.n_rho, w.rho_max, w.threshold, w.window, max_peaks=w.max_peaks, acc_dtype=w.acc_dtype,
@@ -272,6 +272,15 @@ class Workbench:
         c = self.out["counts"].cpu()
         return int(c[:, 1].sum().item()), int(c[:, 0].clamp(max=self.w.max_peaks).sum().item())
 
+    def retention(self):
+        """The paper's two quality figures on the synthetic events (context, not a parity claim): data compression ratio
+        R_c = N_select / N_total (Eq. (8)) and signal retention ratio R_s = N_true,select / N_true
+        (Eq. (9)), N_true = the generator's signal-track hits."""
+        keep = self.out["keep"].cpu().numpy().astype(bool)
+        sig = self.truth.astype(bool)
+        return {"R_c": float(keep.mean()) if keep.size else None, "R_s": float(keep[sig].mean()) if sig.any() else None,
+                "signal_hit_fraction": float(sig.mean()) if sig.size else None}
+
     def alg_bytes(self, counts=None):
         n_kept, n_peaks = counts if counts is not None else self.counts()
         return 8 * self.n_total + 4 * (self.n_events + 1) + self.n_total + 12 * n_kept + 8 * n_peaks + 8 * self.n_events
@@ -305,7 +314,7 @@ def config_line(wb, times_ms, v_in, v_in_how, atom_rate, hbm_gbs, hbm_src):
             "cluster_size": wb.info["CLUSTER_SIZE"], "threads": wb.info["THREADS"], "ctas_per_sm": wb.info["CTAS_PER_SM"],
             "steps": int(len(times_ms)), "ms_per_step": ms, "ms_per_step_min": float(times_ms.min()), "ms_per_step_median": float(np.median(times_ms)),
             "events_per_s": wb.n_events / t, "gvotes_per_s": wb.pairs / t / 1e9, "gvotes_in_range_per_s": v_in / t / 1e9,
-            "frac": r["frac"], "hbm_frac": r["hbm"]["frac"], "kept_fraction": n_kept / max(1, wb.n_total)}
+            "frac": r["frac"], "hbm_frac": r["hbm"]["frac"], "kept_fraction": n_kept / max(1, wb.n_total), "quality": wb.retention()}
 
 
 def multi_stream_sweep(wb, torch, batches=(1000, 10000, 100000), streams_list=(1, 2, 4), reps=3):
@@ -419,6 +428,7 @@ def run_ours(args):
     # ---- what the roofline needs from the device, gathered before anything else runs (untimed)
     v_in, v_in_how = wb.in_range_votes(None if n_events <= 5000 else 2000)
     alg_counts = wb.counts()
+    quality = wb.retention()
     atom_rate = hb.hough_bench_shared_atomics(5, 1, 1024, 20000)          # conflict-free ATOMS/s, all SMs, measured now
     probe = hb.hough_bench_vote_loop(15, 6, 2, 512, 20)                   # the voting loop's instruction sequence alone
 
@@ -503,7 +513,7 @@ def run_ours(args):
             "l2": "cold: 256 MiB write between steps" if flush is not None else "warm",
             "hits_per_gpu": n_total, "launch": info, "ms_per_step_warm_l2_back_to_back": warm_ms,
             "ms_per_step_min": float(times.min()), "ms_per_step_median": float(np.median(times)),
-            "kept_fraction": alg_counts[0] / max(1, n_total), "wall_s_timed_region": t_wall}),
+            "kept_fraction": alg_counts[0] / max(1, n_total), "quality": quality, "wall_s_timed_region": t_wall}),
         "gvotes_per_s": world * wb.pairs / t_kernel / 1e9,
         "gvotes_in_range_per_s": world * v_in / t_kernel / 1e9,
         "roofline": roof, "clocks": clocks,

@@ -64,6 +64,8 @@ def parse_args():
     ap.add_argument("--no-all-configs", action="store_true", help="skip the all_configs / multi_stream blocks (headline only)")
     ap.add_argument("--config-steps", type=int, default=20, help="timed steps per configuration in the all_configs block")
     ap.add_argument("--sweep-events", type=int, default=100000, help="events of the config-4 sweep (all_configs, multi_stream)")
+    ap.add_argument("--segment", default="", choices=["", "probes"],
+                    help="internal: run one side measurement in this (child) process and print its JSON")
     return ap.parse_args()
 
 
@@ -205,6 +207,52 @@ def hbm_peak():
         return 6650.0, "fallback (B200_PROFILING.md)"
 
 
+def run_probe_segment():
+    """Child process of device_probes(): the two measurement aids of include/hough_bench.h on this rank's GPU, each
+    guarded, one JSON object on stdout."""
+    import torch
+    import paper_2607_04067_b200 as hb
+    _, local_rank, _ = dist_env()
+    torch.cuda.set_device(local_rank)
+    torch.zeros(1, device=torch.device("cuda", local_rank))
+    out = {}
+    for key, call in (("atom_rate", lambda: hb.hough_bench_shared_atomics(5, 1, 1024, 20000)),      # conflict-free ATOMS/s, all SMs
+                      ("vote_loop", lambda: hb.hough_bench_vote_loop(15, 6, 2, 512, 20))):          # the voting loop's instruction sequence alone
+        try:
+            out[key] = float(call())
+        except Exception as ex:  # noqa: BLE001
+            out[key + "_error"] = "%s: %s" % (type(ex).__name__, ex)
+    print(json.dumps(out), flush=True)
+    return 0
+
+
+def device_probes(sm_count, sm_max_mhz, timeout_s=300):
+    """The roofline's denominator (hough_bench_shared_atomics(5)) and the vote-loop probe, measured now, in a process
+    of their own: the measurement aids are not product code, and a failure in them (even one that loses the CUDA
+    context) must not cost the headline.  If the measurement fails the peak is the derived one -- 32 shared atomics
+    per clock per SM (one per lane per issue) x SMs x the maximum SM clock -- and says so."""
+    import subprocess
+    res, err = {}, None
+    try:
+        r = subprocess.run([sys.executable, os.path.abspath(__file__), "--segment", "probes"], capture_output=True, text=True,
+                           timeout=timeout_s, cwd=ROOT)
+        lines = [l for l in r.stdout.splitlines() if l.startswith("{")]
+        if lines:
+            res = json.loads(lines[-1])
+        else:
+            err = "probe process exited %s: %s" % (r.returncode, (r.stderr or "").strip().splitlines()[-1:] or "no output")
+    except Exception as ex:  # noqa: BLE001
+        err = "%s: %s" % (type(ex).__name__, ex)
+    atom_rate, probe = res.get("atom_rate"), res.get("vote_loop")
+    if atom_rate and atom_rate > 0:
+        src = "hough_bench_shared_atomics(variant 5) measured in this run: conflict-free 32-bit shared atomics, all SMs"
+    else:
+        atom_rate = 32.0 * (sm_count or 148) * (sm_max_mhz or 1965) * 1e6
+        src = ("DERIVED, not measured: 32 shared atomics per clock per SM x %d SMs x %d MHz (the live measurement failed: %s)"
+               % (sm_count or 148, sm_max_mhz or 1965, err or res.get("atom_rate_error")))
+    return atom_rate, src, (probe if probe and probe > 0 else None), (None if probe else err or res.get("vote_loop_error"))
+
+
 class Workbench:
     """One workload resident on the device: inputs, outputs, handle.  Marshalling and timing only."""
 
@@ -289,7 +337,7 @@ class Workbench:
         self.h.close()
 
 
-def roofline_block(wb, t_kernel_s, v_in, v_in_how, atom_rate, hbm_gbs, hbm_src, counts=None):
+def roofline_block(wb, t_kernel_s, v_in, v_in_how, atom_rate, hbm_gbs, hbm_src, counts=None, atom_src=None):
     alg_bytes = wb.alg_bytes(counts)
     t_vote, t_hbm = v_in / atom_rate, alg_bytes / (hbm_gbs * 1e9)
     return {
@@ -297,7 +345,7 @@ def roofline_block(wb, t_kernel_s, v_in, v_in_how, atom_rate, hbm_gbs, hbm_src, 
         "achieved": v_in / t_kernel_s / 1e9, "peak": atom_rate / 1e9, "unit": "Gvotes/s (in-range)",
         "frac": max(t_vote, t_hbm) / t_kernel_s,
         "traffic": None, "traffic_note": "no ncu capture of this commit in this run; see profiles/ for the last one and its commit",
-        "peak_source": "hough_bench_shared_atomics(variant 5) measured in this run: conflict-free 32-bit shared atomics, all SMs",
+        "peak_source": atom_src or "hough_bench_shared_atomics(variant 5) measured in this run: conflict-free 32-bit shared atomics, all SMs",
         "algorithmic_votes_per_launch": v_in, "votes_counted": v_in_how, "algorithmic_bytes_per_launch": alg_bytes,
         "t_vote_us": t_vote * 1e6, "t_hbm_us": t_hbm * 1e6, "t_kernel_us": t_kernel_s * 1e6,
         "hbm": {"achieved": alg_bytes / t_kernel_s / 1e9, "peak": hbm_gbs, "unit": "GB/s", "frac": t_hbm / t_kernel_s, "peak_source": hbm_src},
@@ -429,8 +477,8 @@ def run_ours(args):
     v_in, v_in_how = wb.in_range_votes(None if n_events <= 5000 else 2000)
     alg_counts = wb.counts()
     quality = wb.retention()
-    atom_rate = hb.hough_bench_shared_atomics(5, 1, 1024, 20000)          # conflict-free ATOMS/s, all SMs, measured now
-    probe = hb.hough_bench_vote_loop(15, 6, 2, 512, 20)                   # the voting loop's instruction sequence alone
+    # the measurement aids run in a process of their own (this one is idle meanwhile): see device_probes()
+    atom_rate, atom_src, probe, probe_err = device_probes(info["SM_COUNT"], clocks.get("sm_max_mhz"))
 
     # ---- end to end through hough_run_host: pinned host buffers, copies inside the timed region.
     # "lean" (headline e2e): H2D hits + offsets, D2H mask + peaks + counts -- what a host consumer that still holds its
@@ -443,20 +491,30 @@ def run_ours(args):
     h_kidx = torch.empty(n_total, dtype=torch.int32).pin_memory()
     e2e_steps = min(args.steps, 50)
     e2e = {}
+    e2e_err = {}
     for mode, kx, ki in (("lean", None, None), ("full", h_kxy, h_kidx)):
-        for _ in range(3):
-            hb.hough_run_host(h.ctx, h_xy, h_off, n_events, h_keep, h_peaks, h_counts, kx, ki, stream)
-        torch.cuda.synchronize()
-        barrier()
         ms_sum = 0.0
-        for _ in range(e2e_steps):
-            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-            a.record(stream)
-            hb.hough_run_host(h.ctx, h_xy, h_off, n_events, h_keep, h_peaks, h_counts, kx, ki, stream)
-            b.record(stream)
-            b.synchronize()               # the caller reads the results on the host here
-            ms_sum += a.elapsed_time(b)
-        barrier()
+        try:      # an error here is reported in the line's e2e block; it must not cost the device-resident headline
+            for _ in range(3):
+                hb.hough_run_host(h.ctx, h_xy, h_off, n_events, h_keep, h_peaks, h_counts, kx, ki, stream)
+            torch.cuda.synchronize()
+            barrier()
+            for _ in range(e2e_steps):
+                a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                a.record(stream)
+                hb.hough_run_host(h.ctx, h_xy, h_off, n_events, h_keep, h_peaks, h_counts, kx, ki, stream)
+                b.record(stream)
+                b.synchronize()               # the caller reads the results on the host here
+                ms_sum += a.elapsed_time(b)
+            barrier()
+            # the host results must be the device-resident run's (same inputs): a cheap end-to-end sanity check, untimed
+            if int(h_counts[:, 1].sum().item()) != alg_counts[0] or int(h_keep.sum().item()) != alg_counts[0]:
+                raise RuntimeError("hough_run_host returned %d kept hits (mask %d), the device-resident run %d"
+                                   % (int(h_counts[:, 1].sum().item()), int(h_keep.sum().item()), alg_counts[0]))
+        except Exception as ex:  # noqa: BLE001
+            if world > 1:
+                raise                          # ranks must stay in step: no partial line under torchrun
+            ms_sum, e2e_err[mode] = float("nan"), "%s: %s" % (type(ex).__name__, ex)
         d2h = h_keep.numel() + h_peaks.numel() * 4 + h_counts.numel() * 4 + (0 if kx is None else h_kxy.numel() * 4 + h_kidx.numel() * 4)
         e2e[mode] = (ms_sum, d2h)
     h2d = h_xy.numel() * 4 + h_off.numel() * 4
@@ -499,11 +557,11 @@ def run_ours(args):
     # ---- roofline of the one kernel (per launch, this rank)
     hbm_gbs, hbm_src = hbm_peak()
     t_kernel = ms_per_step * 1e-3
-    roof = roofline_block(wb, t_kernel, v_in, v_in_how, atom_rate, hbm_gbs, hbm_src, counts=alg_counts)
+    roof = roofline_block(wb, t_kernel, v_in, v_in_how, atom_rate, hbm_gbs, hbm_src, counts=alg_counts, atom_src=atom_src)
     # diagnostic third ceiling: the voting loop's own instruction sequence, alone on the SMs, measured now
     roof["vote_loop_probe"] = {"lane_votes_per_s_incl_padding": probe, "unit": "hit x theta pairs/s, 192 padded columns per 180",
-                               "kernel_vs_probe": (wb.pairs * 192.0 / 180.0 / t_kernel) / probe if w.n_theta == 180 else None,
-                               "probe_vs_atomic_peak": probe / atom_rate}
+                               "kernel_vs_probe": (wb.pairs * 192.0 / 180.0 / t_kernel) / probe if probe and w.n_theta == 180 else None,
+                               "probe_vs_atomic_peak": probe / atom_rate if probe else None, "error": probe_err}
 
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
@@ -517,11 +575,13 @@ def run_ours(args):
         "gvotes_per_s": world * wb.pairs / t_kernel / 1e9,
         "gvotes_in_range_per_s": world * v_in / t_kernel / 1e9,
         "roofline": roof, "clocks": clocks,
-        "e2e": {"value": shard.job_throughput(n_events, world, e2e_lean_ms / e2e_steps), "unit": UNIT,
-                "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": e2e["lean"][1], "ms_per_step": e2e_lean_ms / e2e_steps, "steps": e2e_steps,
+        "e2e": {"value": None if "lean" in e2e_err else shard.job_throughput(n_events, world, e2e_lean_ms / e2e_steps), "unit": UNIT,
+                "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": e2e["lean"][1],
+                "ms_per_step": None if "lean" in e2e_err else e2e_lean_ms / e2e_steps, "steps": e2e_steps, "error": e2e_err.get("lean"),
                 "returns": "keep mask + peaks + counts (lean mode of hough_run_host)",
-                "full": {"value": shard.job_throughput(n_events, world, e2e_full_ms / e2e_steps), "d2h_bytes_per_step": e2e["full"][1],
-                         "ms_per_step": e2e_full_ms / e2e_steps, "returns": "lean + kept_xy + kept_idx (full-length arrays)"},
+                "full": {"value": None if "full" in e2e_err else shard.job_throughput(n_events, world, e2e_full_ms / e2e_steps),
+                         "d2h_bytes_per_step": e2e["full"][1], "ms_per_step": None if "full" in e2e_err else e2e_full_ms / e2e_steps,
+                         "error": e2e_err.get("full"), "returns": "lean + kept_xy + kept_idx (full-length arrays)"},
                 "overlapped_4_streams": {"value": None if e2e_ov_err else shard.job_throughput(n_events, world, e2e_ov_ms / e2e_steps),
                                          "ms_per_step": None if e2e_ov_err else e2e_ov_ms / e2e_steps, "error": e2e_ov_err,
                                          "what": "the lean transfer as 4 sub-batches on 4 streams, one staging area per stream (PAPER.md:228)"}},
@@ -572,6 +632,8 @@ def run_ours(args):
 
 def main():
     args = parse_args()
+    if args.segment == "probes":
+        return run_probe_segment()
     if args.impl == "reference":
         return run_reference(args)
     return run_ours(args)

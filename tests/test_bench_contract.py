@@ -62,3 +62,17 @@ def test_default_arguments_and_blocks_of_the_gpu_arm():
     for key in ('"roofline"', '"cpu_baseline"', '"e2e"', '"all_configs"', '"multi_stream"', '"gpu_launches"', '"clocks"'):
         assert key in src, key
     assert "_work" not in src and "/root/reference" not in src
+
+
+def test_probe_segment_failure_falls_back_to_the_derived_peak_and_says_so():
+    """The roofline denominator is measured in a child process; when that fails (here: no GPU) the line still carries a
+    peak -- the derived 32 atomics per clock per SM -- and its source says it was not measured."""
+    import torch
+    if torch.cuda.is_available():
+        import pytest
+        pytest.skip("a GPU is present")
+    sys.path.insert(0, ROOT)
+    import bench
+    rate, src, probe, probe_err = bench.device_probes(148, 1965, timeout_s=600)
+    assert rate == 32.0 * 148 * 1965e6
+    assert src.startswith("DERIVED, not measured") and probe is None and probe_err

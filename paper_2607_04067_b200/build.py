@@ -15,6 +15,9 @@ import os
 import re
 import subprocess
 import sys
+import threading
+
+_BUILD_LOCK = threading.Lock()      # one build at a time per process (the temporary file is named after the pid)
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
@@ -117,6 +120,11 @@ def check_bench_sass(lib: str = BENCH_LIB) -> dict:
 
 
 def build(flavor: str = "release", force: bool = False, verbose: bool = False) -> str:
+    with _BUILD_LOCK:
+        return _build_locked(flavor, force, verbose)
+
+
+def _build_locked(flavor: str, force: bool, verbose: bool) -> str:
     lib = lib_path(flavor)
     if not force and not _stale(flavor):
         return lib

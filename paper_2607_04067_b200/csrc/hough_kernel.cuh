@@ -126,9 +126,9 @@ __device__ __forceinline__ void circle_of(float cj, float sj, int k, float inv, 
 
 // ---------------------------------------------------------------- small helpers
 #ifdef HOUGH_HOST_EMU
-inline void red_shared_add(unsigned saddr, unsigned v) { *(unsigned*)emu::shared_ptr(saddr) += v; }
-inline void vote_add(unsigned saddr, unsigned v) { *(unsigned*)emu::shared_ptr(saddr) += v; }
-inline void red_shared_or(unsigned saddr, unsigned v) { *(unsigned*)emu::shared_ptr(saddr) |= v; }
+inline void red_shared_add(unsigned saddr, unsigned v) { __atomic_fetch_add((unsigned*)emu::shared_ptr(saddr), v, __ATOMIC_RELAXED); }
+inline void vote_add(unsigned saddr, unsigned v) { __atomic_fetch_add((unsigned*)emu::shared_ptr(saddr), v, __ATOMIC_RELAXED); }
+inline void red_shared_or(unsigned saddr, unsigned v) { __atomic_fetch_or((unsigned*)emu::shared_ptr(saddr), v, __ATOMIC_RELAXED); }
 #else
 __device__ __forceinline__ void red_shared_add(unsigned saddr, unsigned v) {
     asm volatile("red.shared.add.u32 [%0], %1;" ::"r"(saddr), "r"(v) : "memory");
@@ -151,19 +151,21 @@ __device__ __forceinline__ void red_shared_or(unsigned saddr, unsigned v) {
 inline void mbar_init(unsigned, unsigned) {}
 inline void fence_proxy_async() {}
 inline void mbar_expect_tx(unsigned, unsigned) {}
-inline void bulk_copy_g2s(unsigned dst, const void* src, unsigned bytes, unsigned bar) {
+EMU_NOSAN inline void bulk_copy_g2s(unsigned dst, const void* src, unsigned bytes, unsigned bar) {
     emu::bulk_check(dst, src, bytes);
     memcpy(emu::shared_ptr(dst), src, bytes);
     emu::mbar_complete(bar);
+    emu::async_write(emu::shared_ptr(dst), bytes, bar);      // race check: written by the copy engine, visible through `bar`
 }
 inline bool mbar_try_wait(unsigned bar, unsigned parity) { return emu::mbar_wait_parity(bar, parity); }
 inline void prefetch_l2_bulk(const void*, unsigned) {}
 // cluster launch control: the emulator hands out the not-yet-launched CTAs of the grid (emu::clc_steal)
-inline void clc_try_cancel(unsigned resp, unsigned bar) {
+EMU_NOSAN inline void clc_try_cancel(unsigned resp, unsigned bar) {
     int* r = (int*)emu::shared_ptr(resp);
     const int id = emu::clc_steal();
     r[0] = id; r[1] = 0; r[2] = 0; r[3] = id >= 0 ? 1 : 0;
     emu::mbar_complete(bar);
+    emu::async_write(r, 16, bar);                            // race check: written by the hardware, visible through `bar`
 }
 inline int clc_query(unsigned resp) {        // the stolen CTA's blockIdx.x, or -1 when nothing was left to steal
     const int* r = (const int*)emu::shared_ptr(resp);
@@ -279,7 +281,7 @@ __device__ __forceinline__ int bin_exact(float u, float v, float c, float s, flo
 }
 
 // Exclusive scan of one int per thread over the CTA; `total` is returned to every thread.
-// wsum: 33 ints of shared scratch.  Contains two __syncthreads().
+// wsum: 33 ints of shared scratch.  Contains two __syncthreads(); may be called back to back.
 __device__ __forceinline__ int block_exscan(int v, int* wsum, int& total) {
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarps = (blockDim.x + 31) >> 5;
     int inc = v;
@@ -288,6 +290,7 @@ __device__ __forceinline__ int block_exscan(int v, int* wsum, int& total) {
         int o = __shfl_up_sync(0xffffffffu, inc, d);
         if (lane >= d) inc += o;
     }
+    __syncwarp();                        // a previous call's reads of wsum[warp] by this warp's lanes come before the write
     if (lane == 31) wsum[warp] = inc;
     __syncthreads();
     if (warp == 0) {
@@ -917,13 +920,14 @@ __global__ void __launch_bounds__(1024, 1) hough_event_kernel(const __grid_const
                 for (int dj = -p.window; dj <= p.window; ++dj) {
                     int j = ((int)pk.theta_bin + dj) % p.n_theta;
                     if (j < 0) j += p.n_theta;
-                    if (HB_CHK(j >= 0 && j < p.n_theta, HB_H6_SETUP)) colq[j] = 1;
+                    if (HB_CHK(j >= 0 && j < p.n_theta, HB_H6_SETUP)) atomicOr(&colq[j], 1);
                 }
                 continue;
             }
+            // (atomic: the windows of two peaks overlap, and two plain stores of the same 1 are still a write-write hazard)
             const int jlo = max(0, (int)pk.theta_bin - p.window), jhi = min(p.n_theta - 1, (int)pk.theta_bin + p.window);
             for (int j = jlo; j <= jhi; ++j)
-                if (HB_CHK(j >= 0 && j < p.n_theta, HB_H6_SETUP)) colq[j] = 1;
+                if (HB_CHK(j >= 0 && j < p.n_theta, HB_H6_SETUP)) atomicOr(&colq[j], 1);
         }
         __syncthreads();
         // number the marked columns (order irrelevant for the OR of S5)

@@ -9,6 +9,7 @@ import os
 import struct
 import subprocess
 import tempfile
+import threading
 
 import numpy as np
 
@@ -23,24 +24,96 @@ SOURCES = [os.path.join(HERE, "emu_main.cpp"), os.path.join(HERE, "simt_shim.h")
 FLAGS = ["-O1", "-g", "-std=c++17", "-ffp-contract=off", "-fno-fast-math", "-DHOUGH_HOST_EMU", "-Wno-unused-variable"]
 
 
-def exe_path(debug_bounds: bool) -> str:
-    return os.path.join(HERE, "hough_emu_dbg" if debug_bounds else "hough_emu")
+def exe_path(debug_bounds: bool, race: bool = False) -> str:
+    return os.path.join(HERE, "hough_emu_race" if race else "hough_emu_dbg" if debug_bounds else "hough_emu")
 
 
-def build(debug_bounds: bool = False, force: bool = False) -> str:
-    exe = exe_path(debug_bounds)
+def _compile(exe: str, extra, race: bool) -> None:
+    if not race:
+        subprocess.check_call(["g++", *FLAGS, *extra, "-o", exe, SOURCES[0]])
+        return
+    # the race-check build: the compiler's -fsanitize=thread instrumentation, linked WITHOUT ThreadSanitizer's runtime
+    # (the hooks are in simt_shim.h); no PIE, so that the reported code addresses can be looked up with addr2line
+    obj = exe + ".o"
+    subprocess.check_call(["g++", *FLAGS, *extra, "-fsanitize=thread", "-no-pie", "-c", "-o", obj, SOURCES[0]])
+    subprocess.check_call(["g++", "-no-pie", "-o", exe, obj])
+    os.remove(obj)
+
+
+_BUILD_LOCK = threading.Lock()
+
+
+def build(debug_bounds: bool = False, force: bool = False, race: bool = False) -> str:
+    with _BUILD_LOCK:
+        return _build_locked(debug_bounds, force, race)
+
+
+def _build_locked(debug_bounds: bool, force: bool, race: bool) -> str:
+    exe = exe_path(debug_bounds, race)
     if not force and os.path.exists(exe) and all(os.path.getmtime(s) <= os.path.getmtime(exe) for s in SOURCES):
         return exe
     tmp = exe + ".tmp.%d" % os.getpid()
-    subprocess.check_call(["g++", *FLAGS, *(["-DHOUGH_DEBUG_BOUNDS"] if debug_bounds else []), "-o", tmp, SOURCES[0]])
+    _compile(tmp, ["-DHOUGH_DEBUG_BOUNDS"] if debug_bounds and not race else [], race)
     os.replace(tmp, exe)
     return exe
+
+
+def build_mutant(exe: str, edits, race: bool = True) -> str:
+    """Compiles the emulator against a COPY of the kernel source with `edits` = [(old, new), ...] applied (each `old`
+    must occur exactly once) and writes it to `exe`: the mutation tests of the race check."""
+    src = open(SOURCES[2]).read()
+    for old, new in edits:
+        if src.count(old) != 1:
+            raise ValueError("mutation anchor occurs %d times: %r" % (src.count(old), old))
+        src = src.replace(old, new)
+    src = src.replace('"../../include/hough.h"', '"%s"' % SOURCES[3])
+    hdr = exe + ".cuh"
+    with open(hdr, "w") as f:
+        f.write(src)
+    _compile(exe, ['-DHOUGH_KERNEL_HEADER="%s"' % hdr], race)
+    return exe
+
+
+class RaceReport(RuntimeError):
+    """The race-check build found conflicting accesses that no barrier orders.  .reports: one dict per distinct pair of
+    code locations: {"text": the emulator's line, "now": "function file:line", "earlier": "function file:line"}."""
+
+    def __init__(self, reports):
+        self.reports = reports
+        super().__init__("%d race report(s):\n%s" % (len(reports), "\n".join(
+            "%s\n    now:     %s\n    earlier: %s" % (r["text"], r["now"], r["earlier"]) for r in reports[:6])))
+
+
+def _symbolize(exe: str, pcs):
+    """{pc: "function file:line <- inlined into file:line <- ..."} (addr2line -i: the whole inline chain, innermost first)."""
+    out = subprocess.run(["addr2line", "-e", exe, "-a", "-f", "-C", "-s", "-i", *pcs], capture_output=True, text=True).stdout.splitlines()
+    sym, key, frames = {}, None, []
+    for l in out + ["0x"]:
+        if l.startswith("0x"):
+            if key is not None:
+                sym[key] = " <- ".join("%s %s" % (frames[i][:50], frames[i + 1]) for i in range(0, len(frames) - 1, 2)) or "?"
+            key, frames = "0x%x" % int(l, 16) if len(l) > 2 else None, []
+        else:
+            frames.append(l)
+    return sym
+
+
+def _race_reports(exe: str, stderr: str):
+    import re
+    lines = [l for l in stderr.splitlines() if l.startswith("RACE ")]
+    pcs = sorted({pc for l in lines for pc in re.findall(r"pc (0x[0-9a-f]+)", l)})
+    sym = _symbolize(exe, pcs) if pcs else {}
+    reports = []
+    for l in lines:
+        now, earlier = re.findall(r"pc (0x[0-9a-f]+)", l)
+        reports.append({"text": l, "now": sym.get(now, "?"), "earlier": sym.get(earlier, "?")})
+    return reports
 
 
 def run(xy, off, n_theta, n_rho, rho_max, threshold, window, table, max_peaks=64, acc_dtype="u16", accum=True,
         conformal_scale=1, cluster_size=0, ctas_per_sm=0, vote_path=0, grid_clusters=0, debug_bounds=False, timeout=900,
         peak_mode=0, rel_permille=500, nms_radius=1, theta_wrap=False, keep_mode=0, keep_tol=0.0, b_field=1.0, circles=False,
-        order=None, staging=0, scheduler=0, steals=None):
+        order=None, staging=0, scheduler=0, steals=None, race=False, exe=None):
     """Same arguments and result keys as tests/test_parity_gpu.py::gpu_run."""
     import paper_2607_04067_b200 as hb
     xy = np.ascontiguousarray(xy, dtype=np.float32).reshape(-1, 2)
@@ -75,7 +148,10 @@ def run(xy, off, n_theta, n_rho, rho_max, threshold, window, table, max_peaks=64
         env.pop("HOUGH_EMU_STEALS", None)
         if steals is not None:         # launch control: events a CTA may take over before its requests fail (default: no limit)
             env["HOUGH_EMU_STEALS"] = str(int(steals))
-        r = subprocess.run([build(debug_bounds), fin, fout], capture_output=True, text=True, timeout=timeout, env=env)
+        exe = exe or build(debug_bounds, race=race)
+        r = subprocess.run([exe, fin, fout], capture_output=True, text=True, timeout=timeout, env=env)
+        if race and r.returncode == 66:
+            raise RaceReport(_race_reports(exe, r.stderr))
         if r.returncode != 0:
             raise RuntimeError("hough_emu failed (rc %d): %s" % (r.returncode, r.stderr.strip()[-400:]))
         raw = open(fout, "rb").read()

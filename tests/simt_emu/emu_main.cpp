@@ -8,7 +8,11 @@
 #ifndef HOUGH_HOST_EMU
 #error "build with -DHOUGH_HOST_EMU (tests/simt_emu/__init__.py)"
 #endif
+#ifdef HOUGH_KERNEL_HEADER      // the mutation tests compile a modified copy of the kernel (tests/test_kernel_races.py)
+#include HOUGH_KERNEL_HEADER
+#else
 #include "../../paper_2607_04067_b200/csrc/hough_kernel.cuh"
+#endif
 
 namespace {
 
@@ -79,6 +83,14 @@ int main(int argc, char** argv) {
     memset(b_kxy.ptr, 0, b_kxy.bytes);
     for (int i = 0; i <= n_total; ++i) ((int*)b_kidx.ptr)[i] = -5;
     memset(b_acc.ptr, 0xEE, b_acc.bytes);
+#ifdef EMU_RACE                  // race check: the output buffers (the inputs are only ever read)
+    emu::race::track(b_keep.ptr, b_keep.bytes, false, -1, "keep");
+    emu::race::track(b_peaks.ptr, b_peaks.bytes, false, -1, "peaks");
+    emu::race::track(b_counts.ptr, b_counts.bytes, false, -1, "counts");
+    emu::race::track(b_kxy.ptr, b_kxy.bytes, false, -1, "kept_xy");
+    emu::race::track(b_kidx.ptr, b_kidx.bytes, false, -1, "kept_idx");
+    if (want_accum) emu::race::track(b_acc.ptr, b_acc.bytes, false, -1, "accum_dump");
+#endif
 
     kp = hough::KParams();
     // the buffers END at a guard page; an empty buffer still gets a valid pointer (one spare element in front)
@@ -124,6 +136,10 @@ int main(int argc, char** argv) {
     b_circ.alloc(circ_bytes + sizeof(hough_circle));
     memset(b_circ.ptr, 0xFF, b_circ.bytes);
     if (want_circles && max_peaks > 0) {
+#ifdef EMU_RACE
+        emu::race::new_launch();
+        emu::race::track(b_circ.ptr, b_circ.bytes, false, -1, "circles");
+#endif
         cpar = hough::CParams();
         cpar.xy = kp.xy; cpar.off = kp.off; cpar.n_events = n_events; cpar.peaks = kp.peaks; cpar.counts = kp.counts;
         cpar.out = (hough_circle*)(b_circ.ptr + sizeof(hough_circle)); cpar.cos_t = kp.cos_t; cpar.sin_t = kp.sin_t;
@@ -143,5 +159,8 @@ int main(int argc, char** argv) {
     if (want_accum) fwrite(b_acc.ptr + 4, 1, accum_bytes, o);
     if (want_circles) fwrite(b_circ.ptr + sizeof(hough_circle), 1, circ_bytes, o);
     fclose(o);
+#ifdef EMU_RACE
+    if (emu::race::n_reports) { fprintf(stderr, "%lu race report(s)\n", emu::race::n_reports); return 66; }
+#endif
     return 0;
 }

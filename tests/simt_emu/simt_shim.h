@@ -3,7 +3,21 @@
 // thread of a cluster is a fiber (ucontext); __syncthreads, cluster.sync and the full-mask warp collectives are
 // barriers at which a fiber yields; shared memory is one guarded buffer per CTA; shared atomics are plain
 // read-modify-writes (fibers never run concurrently).  It checks the kernel's LOGIC (indexing, phase order,
-// bounds) against the oracle without a GPU; it says nothing about races, PTX semantics or speed.
+// bounds) against the oracle without a GPU; it says nothing about PTX semantics or speed.
+//
+// Race check (the hough_emu_race build: this file compiled with -fsanitize=thread but linked WITHOUT ThreadSanitizer's
+// runtime).  The compiler's instrumentation calls __tsan_read<N> / __tsan_write<N> / __tsan_atomic* for every memory
+// access of the kernel; the hooks at the end of this file implement a detector made for CUDA's synchronisation: every
+// barrier is all-inclusive at its scope (warp: __syncwarp; CTA: __syncthreads*; cluster: cluster.sync), so an earlier
+// access A happens before a later access B exactly when B's thread has passed more barriers of a scope both share
+// than A's thread had when it made A.  Every thread counts the barriers it has passed, every byte of shared memory
+// (of all CTAs of the cluster) and of the global output buffers remembers its last plain write, its last atomics and
+// the reads since; two accesses of different threads to the same byte, at least one a write and not both atomic,
+// that no barrier orders, are reported with both code addresses.  cp.async.bulk / launch-control writes are "async"
+// writes: ordered after what the issuing thread did before, and before a reader only through the mbarrier phase it
+// waited for.  Threads of different clusters of one launch are never ordered.  This is what compute-sanitizer's
+// racecheck reports for shared memory, extended to DSMEM and global memory.  (Warp shuffles and votes order nothing.
+// The emulator's own bookkeeping is excluded from the instrumentation: EMU_NOSAN.)
 #pragma once
 #include <sys/mman.h>
 #include <ucontext.h>
@@ -16,6 +30,13 @@
 #include <cstring>
 #include <utility>
 #include <vector>
+
+#if defined(__SANITIZE_THREAD__)
+#define EMU_RACE 1
+#define EMU_NOSAN __attribute__((no_sanitize("thread")))
+#else
+#define EMU_NOSAN
+#endif
 
 #define __global__
 #define __device__
@@ -87,10 +108,12 @@ struct Cta {
 
 struct Fiber {
     ucontext_t ctx;
-    std::vector<unsigned char> stack;
+    unsigned char* stack = nullptr;  // a slice of run_cluster's one stack block
     dim3 tidx;
     Cta* cta = nullptr;
     bool done = false;
+    // race check: who this is, and how many barriers of each scope it has passed (see the header comment)
+    unsigned fid = 0, cta_uid = 0, cl_gen = 0, cta_gen = 0, warp_gen = 0, mbar_seen[2] = {0, 0};
     unsigned long progress = 0;      // bumped whenever the fiber gets past a wait
 };
 
@@ -106,12 +129,124 @@ struct Grid {
 inline Grid g;
 inline Fiber* cur = nullptr;
 
-inline void yield() {
+#ifdef EMU_RACE
+// ---------------------------------------------------------------- race check: shadow state and the ordering rule
+namespace race {
+
+enum Kind : unsigned char { NONE = 0, READ = 1, WRITE = 2, ATOMIC = 3, ASYNC = 4 };
+struct Rec {                                   // one remembered access of one byte
+    unsigned fid = 0, cl = 0, cta = 0, wg = 0, pc = 0, mphase = 0;
+    unsigned short cta_uid = 0;
+    unsigned char kind = NONE, mslot = 0;
+};
+struct Shadow { Rec w, a[2], r[3]; };          // last plain / async write, last atomics (two threads), reads since (three threads)
+struct Region {
+    unsigned char* lo = nullptr;
+    size_t bytes = 0;
+    bool shared = false;
+    int rank = 0;
+    const char* name = "";
+    std::vector<Shadow> sh;
+};
+inline std::vector<Region> regions;
+inline unsigned long n_reports = 0;
+inline std::vector<unsigned long long> seen_pairs;
+
+EMU_NOSAN inline void track(void* p, size_t bytes, bool shared, int rank, const char* name = "shared") {
+    regions.emplace_back();
+    Region& r = regions.back();
+    r.lo = (unsigned char*)p; r.bytes = bytes; r.shared = shared; r.rank = rank; r.name = name;
+    r.sh.assign(bytes, Shadow());
+}
+EMU_NOSAN inline void untrack_shared() {       // shared memory dies with its cluster
+    for (size_t i = regions.size(); i-- > 0;)
+        if (regions[i].shared) regions.erase(regions.begin() + (long)i);
+}
+EMU_NOSAN inline void new_launch() {           // a kernel boundary orders everything: forget the global history
+    for (auto& r : regions) r.sh.assign(r.bytes, Shadow());
+}
+
+// does the remembered access `p` happen before whatever the current thread does now?
+EMU_NOSAN inline bool ordered(const Rec& p) {
+    const Fiber* c = cur;
+    const unsigned csz = (unsigned)g.csize;
+    if (p.cta_uid / csz != c->cta_uid / csz) return false;                    // another cluster of the launch: never
+    const bool same_cta = p.cta_uid == c->cta_uid;
+    if (p.kind == ASYNC) return same_cta && c->mbar_seen[p.mslot] >= p.mphase;   // only the mbarrier phase orders an async write
+    if (p.fid == c->fid) return true;                                         // program order
+    if (p.cl < c->cl_gen) return true;
+    if (same_cta && p.cta < c->cta_gen) return true;
+    if (same_cta && (p.fid >> 5) == (c->fid >> 5) && p.wg < c->warp_gen) return true;   // (block sizes are multiples of 32)
+    return false;
+}
+
+EMU_NOSAN inline void report(const Region& rg, size_t off, unsigned char kind, unsigned pc, const Rec& p) {
+    const unsigned long long key = ((unsigned long long)pc << 32) | p.pc;
+    for (auto k : seen_pairs) if (k == key) return;
+    seen_pairs.push_back(key);
+    ++n_reports;
+    static const char* names[] = {"none", "read", "write", "atomic", "async-write"};
+    const unsigned th = (unsigned)g.bdim.x;
+    fprintf(stderr, "RACE %s+%zu (cta rank %d's): %s by cta %u thread %u pc 0x%x  <->  earlier %s by cta %u thread %u pc 0x%x\n",
+            rg.name, off, rg.rank, names[kind], cur->cta_uid, cur->fid % th, pc, names[p.kind], (unsigned)p.cta_uid, p.fid % th, p.pc);
+}
+
+EMU_NOSAN inline void access(const void* addr, size_t size, unsigned char kind, const void* ret_pc, unsigned mslot = 0, unsigned mphase = 0) {
+    static bool busy = false;      // the containers used below are instrumented library code: their accesses are not the kernel's
+    if (!cur || busy) return;                                                  // (!cur: host code -- set-up, read-back)
+    busy = true;
+    struct Done { ~Done() { busy = false; } } done;
+    const unsigned char* a = (const unsigned char*)addr;
+    Region* rg = nullptr;
+    for (auto& r : regions)
+        if (a >= r.lo && a < r.lo + r.bytes) { rg = &r; break; }
+    if (!rg) return;                                                           // stack, parameters, read-only inputs
+    const unsigned pc = (unsigned)(size_t)ret_pc - 1;
+    Rec me;
+    me.fid = cur->fid; me.cl = cur->cl_gen; me.cta = cur->cta_gen; me.wg = cur->warp_gen; me.pc = pc;
+    me.cta_uid = (unsigned short)cur->cta_uid; me.kind = kind; me.mslot = (unsigned char)mslot; me.mphase = mphase;
+    for (size_t i = 0; i < size && (size_t)(a - rg->lo) + i < rg->bytes; ++i) {
+        const size_t off = (size_t)(a - rg->lo) + i;
+        Shadow& s = rg->sh[off];
+        // a plain or async write conflicts with everything; a read with writes and atomics; an atomic with plain accesses
+        if (s.w.kind != NONE && !ordered(s.w)) report(*rg, off, kind, pc, s.w);
+        if (kind != ATOMIC)
+            for (auto& q : s.a) if (q.kind != NONE && !ordered(q)) report(*rg, off, kind, pc, q);
+        if (kind != READ)
+            for (auto& q : s.r) if (q.kind != NONE && !ordered(q)) report(*rg, off, kind, pc, q);
+        if (kind == READ) {
+            // remember this read: replace my own older one or one that is ordered before me (then it is ordered before
+            // every later access too); else take a free slot; else keep reads of different warps
+            Rec* slot = nullptr;
+            for (auto& q : s.r) if (q.kind != NONE && (q.fid == me.fid || ordered(q))) { slot = &q; break; }
+            if (!slot) for (auto& q : s.r) if (q.kind == NONE) { slot = &q; break; }
+            if (!slot && (s.r[0].fid >> 5) == (s.r[1].fid >> 5) && (s.r[0].fid >> 5) != (me.fid >> 5)) slot = &s.r[1];
+            if (!slot && (s.r[1].fid >> 5) == (s.r[2].fid >> 5) && (s.r[1].fid >> 5) != (me.fid >> 5)) slot = &s.r[2];
+            if (slot) *slot = me;
+        } else if (kind == ATOMIC) {
+            Rec* slot = nullptr;
+            for (auto& q : s.a) if (q.kind != NONE && (q.fid == me.fid || ordered(q))) { slot = &q; break; }
+            if (!slot) for (auto& q : s.a) if (q.kind == NONE) { slot = &q; break; }
+            if (!slot) slot = &s.a[(me.fid >> 5) == (s.a[0].fid >> 5) ? 0 : 1];
+            *slot = me;
+            for (auto& q : s.r) q.kind = NONE;                                 // (checked above)
+        } else {
+            s.w = me;
+            for (auto& q : s.a) q.kind = NONE;
+            for (auto& q : s.r) q.kind = NONE;
+        }
+    }
+}
+
+}  // namespace race
+#endif
+
+EMU_NOSAN inline void yield() {
     Fiber* me = cur;
     swapcontext(&me->ctx, &g.sched);
 }
 
-inline void wait_barrier(Barrier& b, int pred, int& r_and, int& r_or, int& r_cnt) {
+EMU_NOSAN inline void wait_barrier(Barrier& b, int pred, int& r_and, int& r_or, int& r_cnt, int scope = 1) {
     const unsigned gen = b.gen;
     b.acc_and &= pred ? 1 : 0;
     b.acc_or |= pred ? 1 : 0;
@@ -125,11 +260,12 @@ inline void wait_barrier(Barrier& b, int pred, int& r_and, int& r_or, int& r_cnt
         while (b.gen == gen) yield();
     }
     ++cur->progress;
+    if (scope == 2) ++cur->cl_gen; else ++cur->cta_gen;      // counted on leaving: by then every thread of the scope has arrived
     r_and = b.res_and; r_or = b.res_or; r_cnt = b.res_cnt;
 }
 
 // full-mask warp collective: every lane deposits `v`, all wait, every lane may read any lane's value
-inline const unsigned* warp_exchange(unsigned v) {
+EMU_NOSAN inline const unsigned* warp_exchange(unsigned v, bool orders_memory = false) {
     Cta* c = cur->cta;
     Warp& w = c->warps[cur->tidx.x >> 5];
     const unsigned gen = w.gen;
@@ -142,24 +278,25 @@ inline const unsigned* warp_exchange(unsigned v) {
         while (w.gen == gen) yield();
     }
     ++cur->progress;
+    if (orders_memory) ++cur->warp_gen;                      // __syncwarp; shuffles and votes order nothing
     return buf;
 }
 
 constexpr unsigned SHARED_WINDOW = 0x01000000u;   // what __cvta_generic_to_shared returns for the first byte
-inline unsigned char* shared_ptr(unsigned saddr) {
+EMU_NOSAN inline unsigned char* shared_ptr(unsigned saddr) {
     const unsigned off = saddr - SHARED_WINDOW;
     if ((size_t)off + 4 > cur->cta->smem.bytes) die("shared-window address outside the CTA's shared memory");
     return cur->cta->smem.ptr + off;
 }
-inline unsigned char* dyn_smem() { return cur->cta->smem.ptr; }
-inline int cluster_id() { return g.cluster; }
-inline int n_clusters() { return g.n_clusters_; }
+EMU_NOSAN inline unsigned char* dyn_smem() { return cur->cta->smem.ptr; }
+EMU_NOSAN inline int cluster_id() { return g.cluster; }
+EMU_NOSAN inline int n_clusters() { return g.n_clusters_; }
 
 // bulk-copy staging: what a cp.async.bulk must satisfy (16-byte aligned source, destination and size; the source inside
 // the hit array)
 inline const unsigned char* bulk_lo = nullptr;
 inline const unsigned char* bulk_hi = nullptr;
-inline void bulk_check(unsigned dst, const void* src, unsigned bytes) {
+EMU_NOSAN inline void bulk_check(unsigned dst, const void* src, unsigned bytes) {
     const unsigned char* s = (const unsigned char*)src;
     if (((size_t)s & 15) || (bytes & 15) || ((dst - SHARED_WINDOW) & 15)) die("cp.async.bulk: source, destination or size not 16-byte aligned");
     if (s < bulk_lo || s + bytes > bulk_hi) die("cp.async.bulk: source range leaves the hit array");
@@ -169,7 +306,7 @@ inline void bulk_check(unsigned dst, const void* src, unsigned bytes) {
 // The CTA's mbarrier: the emulated copy lands at issue time, which completes one phase; a waiter of parity p gets true
 // once the phase of that parity has completed, else it yields (so a thread that runs ahead of the issuing thread really
 // waits, as it does for the asynchronous copy on the device).
-inline unsigned& mbar_slot(unsigned bar) {
+EMU_NOSAN inline unsigned& mbar_slot(unsigned bar) {
     Cta* c = cur->cta;
     for (int i = 0; i < 2; ++i) {
         if (c->mbar_addr[i] == bar) return c->mbar_phases[i];
@@ -177,18 +314,34 @@ inline unsigned& mbar_slot(unsigned bar) {
     }
     die("more than two mbarriers in one CTA");
 }
-inline void mbar_complete(unsigned bar) { ++mbar_slot(bar); }
-inline bool mbar_wait_parity(unsigned bar, unsigned parity) {
-    if ((mbar_slot(bar) & 1u) != (parity & 1u)) { ++cur->progress; return true; }
+EMU_NOSAN inline void mbar_complete(unsigned bar) { ++mbar_slot(bar); }
+EMU_NOSAN inline bool mbar_wait_parity(unsigned bar, unsigned parity) {
+    unsigned& ph = mbar_slot(bar);
+    if ((ph & 1u) != (parity & 1u)) {
+        cur->mbar_seen[&ph - cur->cta->mbar_phases] = ph;     // race check: async writes of the phases up to ph are visible now
+        ++cur->progress;
+        return true;
+    }
     yield();
     return false;
 }
+// race check: a write made by the copy engine / the launch-control hardware on behalf of the current thread; readers see
+// it through the completed phase of mbarrier `bar`
+EMU_NOSAN inline void async_write(void* p, unsigned bytes, unsigned bar) {
+#ifdef EMU_RACE
+    unsigned& ph = mbar_slot(bar);
+    race::access(p, bytes, race::ASYNC, __builtin_return_address(0), (unsigned)(&ph - cur->cta->mbar_phases), ph);
+#else
+    (void)p; (void)bytes; (void)bar;
+#endif
+}
+
 // Cluster launch control: the CTAs of the grid that have not started yet are cluster ids next_unlaunched .. n-1 (the
 // emulator runs one CTA after the other).  A request hands out the next of them -- the hardware then never launches it
 // -- unless this CTA has used up its share (HOUGH_EMU_STEALS, default unlimited; a small number mixes stolen and
 // regularly launched CTAs) or none is left; -1 = the request failed.
 inline int next_unlaunched = 0;
-inline int clc_steal() {
+EMU_NOSAN inline int clc_steal() {
     if (cur->cta->steals_left == 0 || next_unlaunched >= g.n_clusters_) return -1;
     if (cur->cta->steals_left > 0) --cur->cta->steals_left;
     return next_unlaunched++;
@@ -196,14 +349,14 @@ inline int clc_steal() {
 
 inline float ftz(float x) { return std::fpclassify(x) == FP_SUBNORMAL ? std::copysign(0.0f, x) : x; }
 
-inline void fiber_main() {
+EMU_NOSAN inline void fiber_main() {
     g.entry();
     cur->done = true;
     swapcontext(&cur->ctx, &g.sched);
 }
 
 // Runs one cluster (csize CTAs of `threads` threads, `smem_bytes` each) to completion.
-inline void run_cluster(int cluster, int n_clusters, int csize, int threads, size_t smem_bytes, void (*entry)()) {
+EMU_NOSAN inline void run_cluster(int cluster, int n_clusters, int csize, int threads, size_t smem_bytes, void (*entry)()) {
     g.bdim.x = (unsigned)threads;
     g.gdim.x = (unsigned)(n_clusters * csize);
     g.csize = csize; g.cluster = cluster; g.n_clusters_ = n_clusters; g.entry = entry;
@@ -211,10 +364,19 @@ inline void run_cluster(int cluster, int n_clusters, int csize, int threads, siz
     g.cluster_bar = Barrier();
     g.cluster_bar.expected = csize * threads;
     std::vector<Fiber> fibers((size_t)csize * threads);
+#ifdef EMU_RACE
+    const size_t stack_bytes = 128 * 1024;
+#else
+    const size_t stack_bytes = 32 * 1024;
+#endif
+    std::vector<unsigned char> stacks(fibers.size() * stack_bytes);     // one block: one mapping, not one per fiber
     for (int r = 0; r < csize; ++r) {
         Cta& c = g.ctas[r];
         c.smem.alloc(smem_bytes);
         memset(c.smem.ptr, 0xCD, smem_bytes);       // shared memory starts as garbage, as on the device
+#ifdef EMU_RACE
+        race::track(c.smem.ptr, smem_bytes, /*shared=*/true, r);
+#endif
         c.rank = r;
         c.bidx.x = (unsigned)(cluster * csize + r);
         c.bar.expected = threads;
@@ -222,12 +384,14 @@ inline void run_cluster(int cluster, int n_clusters, int csize, int threads, siz
         c.steals_left = getenv("HOUGH_EMU_STEALS") ? atoi(getenv("HOUGH_EMU_STEALS")) : -1;
         for (int t = 0; t < threads; ++t) {
             Fiber& f = fibers[(size_t)r * threads + t];
-            f.stack.resize(32 * 1024);
+            f.stack = stacks.data() + ((size_t)r * threads + t) * stack_bytes;
+            f.fid = (unsigned)((cluster * csize + r) * threads + t);
+            f.cta_uid = (unsigned)(cluster * csize + r);
             f.tidx.x = (unsigned)t;
             f.cta = &c;
             getcontext(&f.ctx);
-            f.ctx.uc_stack.ss_sp = f.stack.data();
-            f.ctx.uc_stack.ss_size = f.stack.size();
+            f.ctx.uc_stack.ss_sp = f.stack;
+            f.ctx.uc_stack.ss_size = stack_bytes;
             f.ctx.uc_link = nullptr;
             makecontext(&f.ctx, (void (*)())fiber_main, 0);
         }
@@ -262,10 +426,41 @@ inline void run_cluster(int cluster, int n_clusters, int csize, int threads, siz
         if (after == before && finished_now == 0) die("deadlock: a barrier or warp collective was not reached by every thread");
     }
     cur = nullptr;
+#ifdef EMU_RACE
+    race::untrack_shared();
+#endif
     for (auto& c : g.ctas) c.smem.release();
 }
 
 }  // namespace emu
+
+#ifdef EMU_RACE
+// ---------------------------------------------------------------- what -fsanitize=thread makes the compiler call
+extern "C" {
+EMU_NOSAN void __tsan_init() {}
+EMU_NOSAN void __tsan_func_entry(void*) {}
+EMU_NOSAN void __tsan_func_exit() {}
+EMU_NOSAN void __tsan_vptr_update(void**, void*) {}
+EMU_NOSAN void __tsan_vptr_read(void**) {}
+#define EMU_HOOK(N)                                                                                                              \
+    EMU_NOSAN void __tsan_read##N(void* p) { emu::race::access(p, N, emu::race::READ, __builtin_return_address(0)); }            \
+    EMU_NOSAN void __tsan_write##N(void* p) { emu::race::access(p, N, emu::race::WRITE, __builtin_return_address(0)); }          \
+    EMU_NOSAN void __tsan_unaligned_read##N(void* p) { emu::race::access(p, N, emu::race::READ, __builtin_return_address(0)); }  \
+    EMU_NOSAN void __tsan_unaligned_write##N(void* p) { emu::race::access(p, N, emu::race::WRITE, __builtin_return_address(0)); }
+EMU_HOOK(1) EMU_HOOK(2) EMU_HOOK(4) EMU_HOOK(8) EMU_HOOK(16)
+#undef EMU_HOOK
+EMU_NOSAN void __tsan_read_range(void* p, unsigned long n) { emu::race::access(p, n, emu::race::READ, __builtin_return_address(0)); }
+EMU_NOSAN void __tsan_write_range(void* p, unsigned long n) { emu::race::access(p, n, emu::race::WRITE, __builtin_return_address(0)); }
+// the kernel's atomics (shim: __atomic builtins, relaxed) arrive here
+#define EMU_ATOMIC(OP, EXPR)                                                                                                     \
+    EMU_NOSAN unsigned __tsan_atomic32_fetch_##OP(volatile unsigned* p, unsigned v, int) {                                       \
+        emu::race::access((const void*)p, 4, emu::race::ATOMIC, __builtin_return_address(0));                                    \
+        const unsigned o = *p; *p = EXPR; return o;                                                                              \
+    }
+EMU_ATOMIC(add, o + v) EMU_ATOMIC(and, o & v) EMU_ATOMIC(or, o | v)
+#undef EMU_ATOMIC
+}
+#endif
 
 // ---------------------------------------------------------------- the CUDA names the kernel uses
 #define threadIdx (emu::cur->tidx)
@@ -274,44 +469,45 @@ inline void run_cluster(int cluster, int n_clusters, int csize, int threads, siz
 #define gridDim (emu::g.gdim)
 #define HOUGH_DYN_SMEM(name) unsigned char* name = emu::dyn_smem()
 
-inline void __syncthreads() { int a, o, c; emu::wait_barrier(emu::cur->cta->bar, 1, a, o, c); }
-inline int __syncthreads_and(int p) { int a, o, c; emu::wait_barrier(emu::cur->cta->bar, p, a, o, c); return a; }
-inline int __syncthreads_or(int p) { int a, o, c; emu::wait_barrier(emu::cur->cta->bar, p, a, o, c); return o; }
-inline int __syncthreads_count(int p) { int a, o, c; emu::wait_barrier(emu::cur->cta->bar, p, a, o, c); return c; }
+EMU_NOSAN inline void __syncthreads() { int a, o, c; emu::wait_barrier(emu::cur->cta->bar, 1, a, o, c); }
+EMU_NOSAN inline int __syncthreads_and(int p) { int a, o, c; emu::wait_barrier(emu::cur->cta->bar, p, a, o, c); return a; }
+EMU_NOSAN inline int __syncthreads_or(int p) { int a, o, c; emu::wait_barrier(emu::cur->cta->bar, p, a, o, c); return o; }
+EMU_NOSAN inline int __syncthreads_count(int p) { int a, o, c; emu::wait_barrier(emu::cur->cta->bar, p, a, o, c); return c; }
 inline void __threadfence() {}
 
-inline void need_full_mask(unsigned m) { if (m != 0xffffffffu) emu::die("only full-mask warp collectives are emulated"); }
-inline int __shfl_sync(unsigned m, int v, int src) { need_full_mask(m); return (int)emu::warp_exchange((unsigned)v)[src & 31]; }
-inline int __shfl_up_sync(unsigned m, int v, int d) {
+EMU_NOSAN inline void need_full_mask(unsigned m) { if (m != 0xffffffffu) emu::die("only full-mask warp collectives are emulated"); }
+EMU_NOSAN inline int __shfl_sync(unsigned m, int v, int src) { need_full_mask(m); return (int)emu::warp_exchange((unsigned)v)[src & 31]; }
+EMU_NOSAN inline int __shfl_up_sync(unsigned m, int v, int d) {
     need_full_mask(m);
     const int lane = (int)(emu::cur->tidx.x & 31);
     const unsigned* b = emu::warp_exchange((unsigned)v);
     return lane >= d ? (int)b[lane - d] : v;
 }
-inline unsigned __ballot_sync(unsigned m, int p) {
+EMU_NOSAN inline unsigned __ballot_sync(unsigned m, int p) {
     need_full_mask(m);
     const unsigned* b = emu::warp_exchange(p ? 1u : 0u);
     unsigned r = 0;
     for (int l = 0; l < 32; ++l) r |= (b[l] & 1u) << l;
     return r;
 }
-inline int __all_sync(unsigned m, int p) { return __ballot_sync(m, p) == 0xffffffffu; }
-inline int __shfl_xor_sync(unsigned m, int v, int d) {
+EMU_NOSAN inline int __all_sync(unsigned m, int p) { return __ballot_sync(m, p) == 0xffffffffu; }
+EMU_NOSAN inline int __shfl_xor_sync(unsigned m, int v, int d) {
     need_full_mask(m);
     const int lane = (int)(emu::cur->tidx.x & 31);
     return (int)emu::warp_exchange((unsigned)v)[(lane ^ d) & 31];
 }
-inline unsigned long long __shfl_xor_sync(unsigned m, unsigned long long v, int d) {
+EMU_NOSAN inline unsigned long long __shfl_xor_sync(unsigned m, unsigned long long v, int d) {
     const unsigned lo = (unsigned)__shfl_xor_sync(m, (int)(unsigned)v, d), hi = (unsigned)__shfl_xor_sync(m, (int)(unsigned)(v >> 32), d);
     return (unsigned long long)lo | ((unsigned long long)hi << 32);
 }
-inline void __syncwarp() { emu::warp_exchange(0u); }
+EMU_NOSAN inline void __syncwarp() { emu::warp_exchange(0u, true); }
 
-inline unsigned atomicAdd(unsigned* p, unsigned v) { unsigned o = *p; *p = o + v; return o; }
-inline int atomicAdd(int* p, int v) { int o = *p; *p = o + v; return o; }
-inline unsigned atomicAnd(unsigned* p, unsigned v) { unsigned o = *p; *p = o & v; return o; }
+inline unsigned atomicAdd(unsigned* p, unsigned v) { return __atomic_fetch_add(p, v, __ATOMIC_RELAXED); }
+inline int atomicAdd(int* p, int v) { return __atomic_fetch_add(p, v, __ATOMIC_RELAXED); }
+inline unsigned atomicAnd(unsigned* p, unsigned v) { return __atomic_fetch_and(p, v, __ATOMIC_RELAXED); }
+inline int atomicOr(int* p, int v) { return __atomic_fetch_or(p, v, __ATOMIC_RELAXED); }
 template <class T> inline T __ldg(const T* p) { return *p; }
-inline size_t __cvta_generic_to_shared(const void* p) {
+EMU_NOSAN inline size_t __cvta_generic_to_shared(const void* p) {
     const ptrdiff_t off = (const unsigned char*)p - emu::cur->cta->smem.ptr;
     if (off < 0 || (size_t)off >= emu::cur->cta->smem.bytes) emu::die("cvta of a pointer outside the CTA's shared memory");
     return (size_t)emu::SHARED_WINDOW + (size_t)off;
@@ -352,9 +548,9 @@ inline unsigned min(unsigned a, int b) { return a < (unsigned)b ? a : (unsigned)
 
 namespace cooperative_groups {
 struct cluster_group {
-    unsigned block_rank() const { return (unsigned)emu::cur->cta->rank; }
-    void sync() const { int a, o, c; emu::wait_barrier(emu::g.cluster_bar, 1, a, o, c); }
-    void* map_shared_rank(void* p, int rank) const {
+    EMU_NOSAN unsigned block_rank() const { return (unsigned)emu::cur->cta->rank; }
+    EMU_NOSAN void sync() const { int a, o, c; emu::wait_barrier(emu::g.cluster_bar, 1, a, o, c, 2); }
+    EMU_NOSAN void* map_shared_rank(void* p, int rank) const {
         const ptrdiff_t off = (unsigned char*)p - emu::cur->cta->smem.ptr;
         if (off < 0 || (size_t)off >= emu::cur->cta->smem.bytes) emu::die("map_shared_rank of a pointer outside shared memory");
         if (rank < 0 || rank >= emu::g.csize) emu::die("map_shared_rank: bad rank");

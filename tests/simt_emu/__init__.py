@@ -148,6 +148,7 @@ def run(xy, off, n_theta, n_rho, rho_max, threshold, window, table, max_peaks=64
         env.pop("HOUGH_EMU_STEALS", None)
         if steals is not None:         # launch control: events a CTA may take over before its requests fail (default: no limit)
             env["HOUGH_EMU_STEALS"] = str(int(steals))
+        race = race or os.environ.get("HOUGH_EMU_RACE") == "1"     # HOUGH_EMU_RACE=1: every emulator test becomes a race check too
         exe = exe or build(debug_bounds, race=race)
         r = subprocess.run([exe, fin, fout], capture_output=True, text=True, timeout=timeout, env=env)
         if race and r.returncode == 66:

@@ -100,13 +100,13 @@ def _symbolize(exe: str, pcs):
 
 def _race_reports(exe: str, stderr: str):
     import re
-    lines = [l for l in stderr.splitlines() if l.startswith("RACE ")]
+    lines = [l for l in stderr.splitlines() if l.startswith("RACE ") or l.startswith("UNINIT ")]
     pcs = sorted({pc for l in lines for pc in re.findall(r"pc (0x[0-9a-f]+)", l)})
     sym = _symbolize(exe, pcs) if pcs else {}
     reports = []
     for l in lines:
-        now, earlier = re.findall(r"pc (0x[0-9a-f]+)", l)
-        reports.append({"text": l, "now": sym.get(now, "?"), "earlier": sym.get(earlier, "?")})
+        found = re.findall(r"pc (0x[0-9a-f]+)", l)
+        reports.append({"text": l, "now": sym.get(found[0], "?"), "earlier": sym.get(found[1], "?") if len(found) > 1 else "-"})
     return reports
 
 
@@ -151,7 +151,7 @@ def run(xy, off, n_theta, n_rho, rho_max, threshold, window, table, max_peaks=64
         race = race or os.environ.get("HOUGH_EMU_RACE") == "1"     # HOUGH_EMU_RACE=1: every emulator test becomes a race check too
         exe = exe or build(debug_bounds, race=race)
         r = subprocess.run([exe, fin, fout], capture_output=True, text=True, timeout=timeout, env=env)
-        if race and r.returncode == 66:
+        if race and (r.returncode == 66 or r.stderr.startswith(("RACE ", "UNINIT "))):      # (a report may be followed by a crash)
             raise RaceReport(_race_reports(exe, r.stderr))
         if r.returncode != 0:
             raise RuntimeError("hough_emu failed (rc %d): %s" % (r.returncode, r.stderr.strip()[-400:]))

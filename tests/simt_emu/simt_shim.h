@@ -16,7 +16,8 @@
 // that no barrier orders, are reported with both code addresses.  cp.async.bulk / launch-control writes are "async"
 // writes: ordered after what the issuing thread did before, and before a reader only through the mbarrier phase it
 // waited for.  Threads of different clusters of one launch are never ordered.  This is what compute-sanitizer's
-// racecheck reports for shared memory, extended to DSMEM and global memory.  (Warp shuffles and votes order nothing.
+// racecheck reports for shared memory, extended to DSMEM and global memory.  The same shadow state gives an initcheck:
+// a read or atomic of a byte that nothing has written since the CTA started (shared) / since the first launch (outputs).  (Warp shuffles and votes order nothing.
 // The emulator's own bookkeeping is excluded from the instrumentation: EMU_NOSAN.)
 #pragma once
 #include <sys/mman.h>
@@ -133,7 +134,7 @@ inline Fiber* cur = nullptr;
 // ---------------------------------------------------------------- race check: shadow state and the ordering rule
 namespace race {
 
-enum Kind : unsigned char { NONE = 0, READ = 1, WRITE = 2, ATOMIC = 3, ASYNC = 4 };
+enum Kind : unsigned char { NONE = 0, READ = 1, WRITE = 2, ATOMIC = 3, ASYNC = 4, PRIOR = 5 };   // PRIOR: written by an earlier launch
 struct Rec {                                   // one remembered access of one byte
     unsigned fid = 0, cl = 0, cta = 0, wg = 0, pc = 0, mphase = 0;
     unsigned short cta_uid = 0;
@@ -162,13 +163,19 @@ EMU_NOSAN inline void untrack_shared() {       // shared memory dies with its cl
     for (size_t i = regions.size(); i-- > 0;)
         if (regions[i].shared) regions.erase(regions.begin() + (long)i);
 }
-EMU_NOSAN inline void new_launch() {           // a kernel boundary orders everything: forget the global history
-    for (auto& r : regions) r.sh.assign(r.bytes, Shadow());
+EMU_NOSAN inline void new_launch() {           // a kernel boundary orders everything: forget the history, keep "was written"
+    for (auto& r : regions)
+        for (auto& s : r.sh) {
+            const bool written = s.w.kind != NONE || s.a[0].kind != NONE || s.a[1].kind != NONE;
+            s = Shadow();
+            if (written) s.w.kind = PRIOR;
+        }
 }
 
 // does the remembered access `p` happen before whatever the current thread does now?
 EMU_NOSAN inline bool ordered(const Rec& p) {
     const Fiber* c = cur;
+    if (p.kind == PRIOR) return true;
     const unsigned csz = (unsigned)g.csize;
     if (p.cta_uid / csz != c->cta_uid / csz) return false;                    // another cluster of the launch: never
     const bool same_cta = p.cta_uid == c->cta_uid;
@@ -208,6 +215,19 @@ EMU_NOSAN inline void access(const void* addr, size_t size, unsigned char kind, 
     for (size_t i = 0; i < size && (size_t)(a - rg->lo) + i < rg->bytes; ++i) {
         const size_t off = (size_t)(a - rg->lo) + i;
         Shadow& s = rg->sh[off];
+        // initcheck: a read (or a read-modify-write) of a byte that nothing has written since the launch / since the CTA
+        // started -- shared memory starts as garbage, the output buffers hold whatever the caller left there
+        if (kind != WRITE && kind != ASYNC && s.w.kind == NONE && s.a[0].kind == NONE && s.a[1].kind == NONE) {
+            const unsigned long long key = ((unsigned long long)pc << 32) | 1u;
+            bool seen = false;
+            for (auto k : seen_pairs) if (k == key) { seen = true; break; }
+            if (!seen) {
+                seen_pairs.push_back(key);
+                ++n_reports;
+                fprintf(stderr, "UNINIT %s+%zu (cta rank %d's): %s of a never-written byte by cta %u thread %u pc 0x%x\n", rg->name, off,
+                        rg->rank, kind == READ ? "read" : "atomic", cur->cta_uid, cur->fid % (unsigned)g.bdim.x, pc);
+            }
+        }
         // a plain or async write conflicts with everything; a read with writes and atomics; an atomic with plain accesses
         if (s.w.kind != NONE && !ordered(s.w)) report(*rg, off, kind, pc, s.w);
         if (kind != ATOMIC)

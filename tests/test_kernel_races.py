@@ -5,7 +5,8 @@ the kernel is checked against the last write, the last atomics and the reads sin
 every CTA of the cluster (DSMEM included) and the global output buffers.  Two accesses of different CUDA threads, at
 least one a write, not both atomic, are a race unless a barrier both threads share lies between them (__syncwarp,
 __syncthreads*, cluster.sync; for cp.async.bulk / launch-control writes: the mbarrier phase the reader waited for).
-Warp shuffles and votes order nothing; threads of different clusters are never ordered.  The mutation tests prove the
+Warp shuffles and votes order nothing; threads of different clusters are never ordered.  The same shadow state gives
+an initcheck: a read or atomic of a byte nothing has written yet is reported too.  The mutation tests prove the
 detector detects: the same scenarios with one barrier removed, or one atomic made a plain store, must be reported at
 the lines involved."""
 import os
@@ -92,6 +93,9 @@ MUTANTS = {
     "block_exscan called back to back without the __syncwarp": (
         [("    __syncwarp();                        // a previous call's reads of wsum[warp]", "    // removed: a previous call's reads of wsum[warp]")],
         dict(cfg=1, nev=1), "wsum[warp]"),
+    "initcheck: the vector-list counter not reset before H4 counts with it": (
+        [("            if (tid == 0) misc[42] = 0;\n        }\n\n        // ---- H0-H3", "        }\n\n        // ---- H0-H3")],
+        dict(cfg=0, nev=1), "misc[42]"),
     "bulk-copy staging: the hits read without waiting for the mbarrier": (
         [("                    bool done = false;\n                    for (int spin = 0; spin < (1 << 24) && !done; ++spin) done = mbar_try_wait(bar_s, bar_phase);",
           "                    bool done = true;")],

@@ -89,7 +89,12 @@ def load_library():
     if _lib is not None:
         return _lib
     path = _build.build(flavor())
-    lib = ctypes.CDLL(path)
+    _lib = _declare_abi(ctypes.CDLL(path))
+    return _lib
+
+
+def _declare_abi(lib):
+    """Argument and result types of every entry point of include/hough.h and include/hough_debug.h."""
     vp, ci, cll = ctypes.c_void_p, ctypes.c_int, ctypes.c_longlong
     lib.hough_create.restype = vp
     lib.hough_create.argtypes = [ci, ci, ctypes.c_float, ci, ci]
@@ -123,7 +128,6 @@ def load_library():
     lib.hough_debug_tame_bounds.argtypes = [ci, ctypes.c_float, ctypes.c_float, ctypes.c_float, ctypes.POINTER(ctypes.c_float)]
     lib.hough_debug_bounds_enabled.restype = ci
     lib.hough_debug_bounds_enabled.argtypes = []
-    _lib = lib
     return lib
 
 

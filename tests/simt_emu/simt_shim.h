@@ -50,7 +50,10 @@
 struct float2 { float x, y; };
 struct float4 { float x, y, z, w; };
 struct alignas(16) uint4 { unsigned x, y, z, w; };
-struct dim3 { unsigned x = 1, y = 1, z = 1; };
+struct dim3 {
+    unsigned x, y, z;
+    dim3(unsigned x_ = 1, unsigned y_ = 1, unsigned z_ = 1) : x(x_), y(y_), z(z_) {}
+};
 inline float2 make_float2(float x, float y) { return float2{x, y}; }
 inline uint4 make_uint4(unsigned x, unsigned y, unsigned z, unsigned w) { return uint4{x, y, z, w}; }
 
@@ -162,6 +165,20 @@ EMU_NOSAN inline void track(void* p, size_t bytes, bool shared, int rank, const 
 EMU_NOSAN inline void untrack_shared() {       // shared memory dies with its cluster
     for (size_t i = regions.size(); i-- > 0;)
         if (regions[i].shared) regions.erase(regions.begin() + (long)i);
+}
+EMU_NOSAN inline void untrack(void* p) {
+    for (size_t i = regions.size(); i-- > 0;)
+        if (regions[i].lo == (unsigned char*)p) regions.erase(regions.begin() + (long)i);
+}
+EMU_NOSAN inline void host_write(void* p, size_t n) {      // a copy or memset between launches: the bytes count as written
+    unsigned char* a = (unsigned char*)p;
+    for (auto& r : regions)
+        if (a >= r.lo && a < r.lo + r.bytes)
+            for (size_t i = 0; i < n && (size_t)(a - r.lo) + i < r.bytes; ++i) {
+                Shadow& s = r.sh[(size_t)(a - r.lo) + i];
+                s = Shadow();
+                s.w.kind = PRIOR;
+            }
 }
 EMU_NOSAN inline void new_launch() {           // a kernel boundary orders everything: forget the history, keep "was written"
     for (auto& r : regions)
@@ -316,10 +333,11 @@ EMU_NOSAN inline int n_clusters() { return g.n_clusters_; }
 // the hit array)
 inline const unsigned char* bulk_lo = nullptr;
 inline const unsigned char* bulk_hi = nullptr;
+inline bool (*bulk_range_ok)(const void*, size_t) = nullptr;      // host emulation: "inside one device allocation"
 EMU_NOSAN inline void bulk_check(unsigned dst, const void* src, unsigned bytes) {
     const unsigned char* s = (const unsigned char*)src;
     if (((size_t)s & 15) || (bytes & 15) || ((dst - SHARED_WINDOW) & 15)) die("cp.async.bulk: source, destination or size not 16-byte aligned");
-    if (s < bulk_lo || s + bytes > bulk_hi) die("cp.async.bulk: source range leaves the hit array");
+    if (bulk_range_ok ? !bulk_range_ok(s, bytes) : (s < bulk_lo || s + bytes > bulk_hi)) die("cp.async.bulk: source range leaves the hit array");
     if ((size_t)(dst - SHARED_WINDOW) + bytes > cur->cta->smem.bytes) die("cp.async.bulk: destination leaves shared memory");
 }
 
@@ -479,14 +497,19 @@ EMU_NOSAN void __tsan_write_range(void* p, unsigned long n) { emu::race::access(
     }
 EMU_ATOMIC(add, o + v) EMU_ATOMIC(and, o & v) EMU_ATOMIC(or, o | v)
 #undef EMU_ATOMIC
+// host code compiled into the same unit (std::atomic counters, the guards of function-local statics): plain operations,
+// the host side of the emulation runs on one thread
+EMU_NOSAN unsigned char __tsan_atomic8_load(const volatile unsigned char* p, int) { return *p; }
+EMU_NOSAN unsigned long long __tsan_atomic64_load(const volatile unsigned long long* p, int) { return *p; }
+EMU_NOSAN unsigned long long __tsan_atomic64_fetch_add(volatile unsigned long long* p, unsigned long long v, int) { const unsigned long long o = *p; *p = o + v; return o; }
 }
 #endif
 
 // ---------------------------------------------------------------- the CUDA names the kernel uses
 #define threadIdx (emu::cur->tidx)
 #define blockIdx (emu::cur->cta->bidx)
-#define blockDim (emu::g.bdim)
-#define gridDim (emu::g.gdim)
+inline dim3& blockDim = emu::g.bdim;      // (objects, not macros: host code has struct members of these names)
+inline dim3& gridDim = emu::g.gdim;
 #define HOUGH_DYN_SMEM(name) unsigned char* name = emu::dyn_smem()
 
 EMU_NOSAN inline void __syncthreads() { int a, o, c; emu::wait_barrier(emu::cur->cta->bar, 1, a, o, c); }

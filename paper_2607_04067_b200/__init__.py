@@ -196,13 +196,18 @@ def hough_set_option_f64(ctx, key, value):
     _check(load_library().hough_set_option_f64(ctx, key, float(value)), "hough_set_option_f64")
 
 
+def _is_device_tensor(t):
+    import torch
+    return isinstance(t, torch.Tensor) and t.is_cuda
+
+
 def hough_circles(ctx, d_xy, d_event_offsets, n_events, d_peaks, d_counts, d_circles, stream=None):
     """d_circles: CUDA uint8 tensor of at least n_events * max_peaks * 48 bytes (hough_circle records)."""
     import torch
     mp = hough_get_info(ctx, HOUGH_INFO_MAX_PEAKS)
     _marshal_check(True, n_events, d_xy, d_event_offsets, None, d_peaks, d_counts, max_peaks=mp)
     if n_events > 0 and mp > 0:
-        if not (isinstance(d_circles, torch.Tensor) and d_circles.is_cuda and d_circles.is_contiguous() and d_circles.dtype == torch.uint8
+        if not (_is_device_tensor(d_circles) and d_circles.is_contiguous() and d_circles.dtype == torch.uint8
                 and d_circles.numel() >= 48 * n_events * mp):
             raise HoughError("d_circles must be a contiguous CUDA uint8 tensor of at least n_events * max_peaks * 48 bytes")
     _check(load_library().hough_circles(ctx, _ptr(d_xy), _ptr(d_event_offsets), n_events, _ptr(d_peaks), _ptr(d_counts),

@@ -20,12 +20,14 @@ void* g_arg = nullptr;
 void entry_event() { ((void (*)(hough::KParams))g_fn)(*(const hough::KParams*)g_arg); }
 void entry_circles() { ((void (*)(hough::CParams))g_fn)(*(const hough::CParams*)g_arg); }
 
+// a bulk copy that starts inside an emulated device allocation must end inside it (memory the fake runtime did not
+// allocate -- a caller's own array in the dry run of the GPU tests -- cannot be judged)
 bool inside_one_allocation(const void* p, size_t n) {
     for (auto& kv : fake_cuda::allocations) {
         const unsigned char* lo = kv.second.ptr;
-        if ((const unsigned char*)p >= lo && (const unsigned char*)p + n <= lo + kv.second.bytes) return true;
+        if ((const unsigned char*)p >= lo && (const unsigned char*)p < lo + kv.second.bytes) return (const unsigned char*)p + n <= lo + kv.second.bytes;
     }
-    return false;
+    return true;
 }
 
 cudaError_t run_grid(const void* fn, void* arg, int grid, int C, int threads, size_t smem, void (*entry)()) {

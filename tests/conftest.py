@@ -48,3 +48,31 @@ def pytest_collection_modifyitems(config, items):
     for item in items:
         if "gpu" in item.keywords:
             item.add_marker(skip)
+
+
+def pytest_collection_finish(session):
+    """The emulator flavours the selected tests will ask for, compiled side by side up front (one g++ each; built one
+    after the other they cost a minute and a half of a fresh checkout's first run)."""
+    wanted = set()
+    for item in session.items:
+        mod = os.path.basename(str(item.fspath))
+        if mod in ("test_kernel_emulation.py", "test_gpu_scenarios_under_emulator.py"):
+            wanted.update(["emu", "emu_dbg"])
+        elif mod == "test_kernel_races.py":
+            wanted.add("emu_race")
+        elif mod == "test_host_emulation.py":
+            wanted.update(["host", "host_race"])
+    if not wanted or session.config.option.collectonly:
+        return
+    from concurrent.futures import ThreadPoolExecutor
+    sys.path.insert(0, os.path.dirname(os.path.abspath(__file__)))
+    import simt_emu
+    from simt_emu import host
+    jobs = {"emu": lambda: simt_emu._build_locked(False, False, False), "emu_dbg": lambda: simt_emu._build_locked(True, False, False),
+            "emu_race": lambda: simt_emu._build_locked(False, False, True), "host": lambda: host._build_unlocked(False),
+            "host_race": lambda: host._build_unlocked(True)}
+    try:
+        with ThreadPoolExecutor(len(wanted)) as ex:
+            list(ex.map(lambda k: jobs[k](), sorted(wanted)))
+    except Exception:  # noqa: BLE001 -- the test that needs the build reports the failure
+        pass

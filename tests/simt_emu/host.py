@@ -22,8 +22,13 @@ _libs = {}
 
 
 def build(race: bool = False, force: bool = False) -> str:
-    lib = os.path.join(HERE, "libhough_hostemu_race.so" if race else "libhough_hostemu.so")
     with _LOCK:
+        return _build_unlocked(race, force)
+
+
+def _build_unlocked(race: bool = False, force: bool = False) -> str:
+    lib = os.path.join(HERE, "libhough_hostemu_race.so" if race else "libhough_hostemu.so")
+    if True:
         if not force and os.path.exists(lib) and all(os.path.getmtime(s) <= os.path.getmtime(lib) for s in HOST_SOURCES):
             return lib
         tmp = lib + ".tmp.%d" % os.getpid()

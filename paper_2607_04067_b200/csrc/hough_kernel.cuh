@@ -478,6 +478,7 @@ __global__ void __launch_bounds__(1024, 1) hough_event_kernel(const __grid_const
         }
 
         // ---- H0-H3: stage, transform, vote (chunked)
+        int ev_tame = 1;                 // every chunk of the event took the packed fast path (CTA-uniform): H6 may take it too
         for (int cbeg = 0; cbeg < n; cbeg += chunk) {
             const int m = min(chunk, n - cbeg);
             int tame = 1;
@@ -504,6 +505,7 @@ __global__ void __launch_bounds__(1024, 1) hough_event_kernel(const __grid_const
                 tame &= ((au >= p.ftz_min || au == 0.0f) && (av >= p.ftz_min || av == 0.0f)) ? 1 : 0;
             }
             const int all_tame = __shfl_sync(0xffffffffu, __syncthreads_and(tame) && !p.force_slow, 0);
+            ev_tame &= all_tame;
             // Every warp votes (nwarps == n_groups * n_stripes).  Hits are dealt in rounds of 2*S:
             // the full rounds have a warp-uniform trip count, which keeps the loop in uniform
             // control flow (shared-window base in a uniform register, ATOMS [R+UR] addressing).
@@ -1015,10 +1017,22 @@ __global__ void __launch_bounds__(1024, 1) hough_event_kernel(const __grid_const
                 const unsigned char* row = W8 + g8 * p.w8_pitch;
                 const float cc[8] = {ca.x, ca.y, ca.z, ca.w, cb.x, cb.y, cb.z, cb.w};
                 const float ss[8] = {sa.x, sa.y, sa.z, sa.w, sb.x, sb.y, sb.z, sb.w};
+                if (ev_tame) {
+                    // two marked columns per packed instruction, as in the voting loop: same six roundings per column,
+                    // same bins for tame hits, 3 FP instructions per column instead of 6
 #pragma unroll
-                for (int i = 0; i < 8; ++i) {
-                    const unsigned k = min(bin_bits(uv.x, uv.y, cc[i], ss[i], rho_max, inv) - HOUGH_MAGIC_BITS, n_rho_u);
-                    hitbits |= (unsigned)row[k] & (1u << i);
+                    for (int i = 0; i < 8; i += 2) {
+                        unsigned b0, b1;
+                        bin_bits2(uv.x, uv.y, pack2(cc[i], cc[i + 1]), pack2(ss[i], ss[i + 1]), rho_max, inv, b0, b1);
+                        const unsigned k0 = min(b0 - HOUGH_MAGIC_BITS, n_rho_u), k1 = min(b1 - HOUGH_MAGIC_BITS, n_rho_u);
+                        hitbits |= ((unsigned)row[k0] & (1u << i)) | ((unsigned)row[k1] & (2u << i));
+                    }
+                } else {
+#pragma unroll
+                    for (int i = 0; i < 8; ++i) {
+                        const unsigned k = min(bin_bits(uv.x, uv.y, cc[i], ss[i], rho_max, inv) - HOUGH_MAGIC_BITS, n_rho_u);
+                        hitbits |= (unsigned)row[k] & (1u << i);
+                    }
                 }
                 if (__all_sync(0xffffffffu, hitbits != 0u || !valid)) break;
             }

@@ -474,11 +474,10 @@ __global__ void __launch_bounds__(1024, 1) hough_event_kernel(const __grid_const
             uint4* z = (uint4*)smem;
             const uint4 zz = make_uint4(0, 0, 0, 0);
             for (int i = tid; i < zero_vec; i += nthreads) z[i] = zz;
-            if (tid == 0) misc[42] = 0;
+            if (tid == 0) { misc[42] = 0; misc[33] = 1; }      // [33]: every chunk of the event took the packed fast path so far
         }
 
         // ---- H0-H3: stage, transform, vote (chunked)
-        int ev_tame = 1;                 // every chunk of the event took the packed fast path (CTA-uniform): H6 may take it too
         for (int cbeg = 0; cbeg < n; cbeg += chunk) {
             const int m = min(chunk, n - cbeg);
             int tame = 1;
@@ -505,7 +504,7 @@ __global__ void __launch_bounds__(1024, 1) hough_event_kernel(const __grid_const
                 tame &= ((au >= p.ftz_min || au == 0.0f) && (av >= p.ftz_min || av == 0.0f)) ? 1 : 0;
             }
             const int all_tame = __shfl_sync(0xffffffffu, __syncthreads_and(tame) && !p.force_slow, 0);
-            ev_tame &= all_tame;
+            if (tid == 0 && !all_tame) misc[33] = 0;      // (kept in shared memory: a register live across the voting loop costs it a reload)
             // Every warp votes (nwarps == n_groups * n_stripes).  Hits are dealt in rounds of 2*S:
             // the full rounds have a warp-uniform trip count, which keeps the loop in uniform
             // control flow (shared-window base in a uniform register, ATOMS [R+UR] addressing).
@@ -988,6 +987,7 @@ __global__ void __launch_bounds__(1024, 1) hough_event_kernel(const __grid_const
 
         // keep test of one hit: OR over the marked columns q of bit q of W8[.][bin(i, column q)]  (== S5)
         const unsigned n_rho_u = (unsigned)p.n_rho;
+        const int ev_tame = misc[33];      // CTA-uniform; written before the chunk's closing barrier
         auto keep_test = [&](float2 uv, float2 h, bool valid) -> bool {
             if (EXT && p.keep_mode == 1) {
                 // N4b: keep iff | ||hit - centre|| - r_c | < tol for some stored peak (fp64, one rounding per operation)

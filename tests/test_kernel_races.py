@@ -94,7 +94,7 @@ MUTANTS = {
         [("    __syncwarp();                        // a previous call's reads of wsum[warp]", "    // removed: a previous call's reads of wsum[warp]")],
         dict(cfg=1, nev=1), "wsum[warp]"),
     "initcheck: the vector-list counter not reset before H4 counts with it": (
-        [("            if (tid == 0) misc[42] = 0;\n        }\n\n        // ---- H0-H3", "        }\n\n        // ---- H0-H3")],
+        [("if (tid == 0) { misc[42] = 0; misc[33] = 1; }", "if (tid == 0) { misc[33] = 1; }")],
         dict(cfg=0, nev=1), "misc[42]"),
     "bulk-copy staging: the hits read without waiting for the mbarrier": (
         [("                    bool done = false;\n                    for (int spin = 0; spin < (1 << 24) && !done; ++spin) done = mbar_try_wait(bar_s, bar_phase);",

@@ -985,7 +985,7 @@ __global__ void __launch_bounds__(1024, 1) hough_event_kernel(const __grid_const
         __syncthreads();
         }   // keep mode
 
-        // keep test of one hit: OR over the marked columns q of bit q of W8[.][bin(i, column q)]  (== S5)
+        // ---- H6 keep test of one hit: OR over the marked columns q of bit q of W8[.][bin(i, column q)]  (== S5)
         const unsigned n_rho_u = (unsigned)p.n_rho;
         const int ev_tame = misc[33];      // CTA-uniform; written before the chunk's closing barrier
         auto keep_test = [&](float2 uv, float2 h, bool valid) -> bool {

@@ -171,6 +171,16 @@ def run(xy, off, n_theta, n_rho, rho_max, threshold, window, table, max_peaks=64
         res["accum"] = take(n_events * n_theta * n_rho, np.int32).reshape(n_events, n_theta, n_rho)
     if circles:
         res["circles"] = take(n_events * max_peaks, CIRCLE_DTYPE).reshape(n_events, max_peaks)
+    if race and env.get("HOUGH_EMU_PROFILE"):       # {(file:line, "shared"|"global", kind): thread-level accesses}
+        import re
+        rows = [l.split() for l in r.stderr.splitlines() if l.startswith("PROF ")]
+        sym = _symbolize(exe, sorted({x[2] for x in rows}))
+        prof = {}
+        for _, _, pc, space, kind, n in rows:
+            m = re.search(r"(hough_kernel\.cuh:\d+)", sym.get(pc, ""))           # the kernel line of the inline chain
+            key = (m.group(1) if m else sym.get(pc, pc), space, kind)
+            prof[key] = prof.get(key, 0) + int(n)
+        res["profile"] = prof
     res["peaks3"] = hb.unpack_peaks(res["peaks"])
     res["info"] = {"CLUSTER_SIZE": plan["cluster_size"], "THREADS": plan["threads"], "SMEM_BYTES": plan["smem_bytes"],
                    "ACC_BITS": plan["acc_bits"], "CHUNK_HITS": plan["chunk_hits"]}

@@ -160,6 +160,9 @@ int main(int argc, char** argv) {
     if (want_circles) fwrite(b_circ.ptr + sizeof(hough_circle), 1, circ_bytes, o);
     fclose(o);
 #ifdef EMU_RACE
+    for (auto& kv : emu::race::profile)
+        fprintf(stderr, "PROF pc 0x%llx %s %s %llu\n", kv.first >> 8, (kv.first & 16) ? "shared" : "global",
+                (const char*[]){"none", "read", "write", "atomic", "async"}[kv.first & 7], kv.second);
     if (emu::race::n_reports) { fprintf(stderr, "%lu race report(s)\n", emu::race::n_reports); return 66; }
 #endif
     return 0;

@@ -29,6 +29,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <map>
 #include <utility>
 #include <vector>
 
@@ -153,6 +154,10 @@ struct Region {
     std::vector<Shadow> sh;
 };
 inline std::vector<Region> regions;
+// HOUGH_EMU_PROFILE=1: how often each code address touched tracked memory, per access kind (dumped by emu_main at exit):
+// a count of the kernel's shared / global memory operations per source line, thread by thread
+inline bool profile_on = getenv("HOUGH_EMU_PROFILE") != nullptr;
+inline std::map<unsigned long long, unsigned long long> profile;      // (pc << 8 | shared << 4 | kind) -> thread-level accesses
 inline unsigned long n_reports = 0;
 inline std::vector<unsigned long long> seen_pairs;
 
@@ -226,6 +231,7 @@ EMU_NOSAN inline void access(const void* addr, size_t size, unsigned char kind, 
         if (a >= r.lo && a < r.lo + r.bytes) { rg = &r; break; }
     if (!rg) return;                                                           // stack, parameters, read-only inputs
     const unsigned pc = (unsigned)(size_t)ret_pc - 1;
+    if (profile_on) ++profile[((unsigned long long)pc << 8) | (rg->shared ? 16u : 0u) | kind];
     Rec me;
     me.fid = cur->fid; me.cl = cur->cl_gen; me.cta = cur->cta_gen; me.wg = cur->warp_gen; me.pc = pc;
     me.cta_uid = (unsigned short)cur->cta_uid; me.kind = kind; me.mslot = (unsigned char)mslot; me.mphase = mphase;

@@ -61,6 +61,7 @@ def parse_args():
                     help="HOUGH_OPT_VOTE_PATH (0 packed fast, 1 exact slow; 2/3 = phase-skipping diagnostics of the bench-only diag build)")
     ap.add_argument("--staging", type=int, default=0, help="HOUGH_OPT_STAGING (0 coalesced loads, 1 cp.async.bulk per chunk)")
     ap.add_argument("--scheduler", type=int, default=0, help="HOUGH_OPT_SCHEDULER (0 one CTA per event, 1 work stealing by cluster launch control)")
+    ap.add_argument("--select", type=int, default=0, help="HOUGH_OPT_SELECT_MODE (0 scan of the marked columns, 1 dense, 2 dense when many peaks)")
     ap.add_argument("--no-all-configs", action="store_true", help="skip the all_configs / multi_stream blocks (headline only)")
     ap.add_argument("--config-steps", type=int, default=20, help="timed steps per configuration in the all_configs block")
     ap.add_argument("--sweep-events", type=int, default=100000, help="events of the config-4 sweep (all_configs, multi_stream)")
@@ -256,7 +257,7 @@ def device_probes(sm_count, sm_max_mhz, timeout_s=300):
 class Workbench:
     """One workload resident on the device: inputs, outputs, handle.  Marshalling and timing only."""
 
-    def __init__(self, hb, si, torch, dev, cfg, n_events, first_event=0, cluster=0, ctas_per_sm=0, vote_path=0, staging=0, scheduler=0):
+    def __init__(self, hb, si, torch, dev, cfg, n_events, first_event=0, cluster=0, ctas_per_sm=0, vote_path=0, staging=0, scheduler=0, select=0):
         self.hb, self.torch, self.dev = hb, torch, dev
         self.w = w = si.config(cfg)
         self.n_events = n_events
@@ -264,7 +265,7 @@ class Workbench:
         self.n_total = len(self.xy)
         self.table = si.trig_table(w.n_theta)
         self.h = hb.Hough(w.n_theta, w.n_rho, w.rho_max, w.threshold, w.window, max_peaks=w.max_peaks, acc_dtype=w.acc_dtype,
-                          cluster_size=cluster, ctas_per_sm=ctas_per_sm, trig_table=self.table, staging=staging, scheduler=scheduler)
+                          cluster_size=cluster, ctas_per_sm=ctas_per_sm, trig_table=self.table, staging=staging, scheduler=scheduler, select_mode=select)
         if vote_path:
             hb.hough_set_option(self.h.ctx, hb.HOUGH_OPT_VOTE_PATH, vote_path)
         self.info = {k: self.h.info(getattr(hb, "HOUGH_INFO_" + k)) for k in
@@ -429,10 +430,10 @@ def run_ours(args):
     n_events = args.events or min(w.n_events, 1000)
     first_event, _ = shard.event_range(rank, world, n_events)             # every rank its own events
     wb = Workbench(hb, si, torch, dev, args.config, n_events, first_event, args.cluster, args.ctas_per_sm, args.vote_path,
-                   args.staging, args.scheduler)
+                   args.staging, args.scheduler, args.select)
     xy, off, n_total, info, h = wb.xy, wb.off, wb.n_total, dict(wb.info), wb.h
     info["VOTE_PATH"] = args.vote_path
-    info["STAGING"], info["SCHEDULER"] = args.staging, args.scheduler      # 0 / 0 = the defaults
+    info["STAGING"], info["SCHEDULER"], info["SELECT_MODE"] = args.staging, args.scheduler, args.select      # 0 / 0 / 0 = the defaults
     info["LIBRARY"] = os.path.basename(hb.lib_path())
     stream = torch.cuda.current_stream()
     flush = None if args.no_flush else torch.empty(256 << 20, dtype=torch.uint8, device=dev)
@@ -594,7 +595,7 @@ def run_ours(args):
         allc = []
         for cfg, nev, cl in ((0, 16, 0), (1, 1000, 0), (2, 1000, 0), (3, 1000, 0), (4, args.sweep_events, 0), (5, args.sweep_events, 0)):
             try:       # a configuration that fails is reported as such; it must not cost the headline line
-                b2 = Workbench(hb, si, torch, dev, cfg, nev, staging=args.staging, scheduler=args.scheduler)
+                b2 = Workbench(hb, si, torch, dev, cfg, nev, staging=args.staging, scheduler=args.scheduler, select=args.select)
                 fl = flush if b2.n_total * 8 < (96 << 20) else None       # inputs larger than L2 need no flush
                 steps2 = args.config_steps if nev <= 1000 else max(5, args.config_steps // 4)
                 t2 = b2.timed(steps2, 3, fl, stream)

@@ -100,13 +100,24 @@ typedef enum hough_option {
                                        1 = one cp.async.bulk (TMA engine) per chunk, completion on an mbarrier, the 16-byte
                                        aligned source range found by aligning down and up by one hit; needs d_xy 16-byte
                                        aligned.  Same results; never yet timed */
-    HOUGH_OPT_SCHEDULER = 13        /* how events reach the SMs (events "assigned to different thread blocks"):
+    HOUGH_OPT_SCHEDULER = 13,       /* how events reach the SMs (events "assigned to different thread blocks"):
                                        0 = one CTA (cluster) per event, dealt by the hardware block scheduler (default);
                                        1 = the same launch, but a resident CTA cancels the launch of a not-yet-started CTA
                                        (Blackwell cluster launch control) and takes over its event, so the per-CTA set-up
                                        runs once per resident CTA, and the next event's hits are prefetched into L2 under
                                        the current event's peak finding and selection; one-CTA-per-event grids only (a
                                        clustered grid ignores it); needs d_xy 16-byte aligned.  Same results; never yet timed */
+    HOUGH_OPT_SELECT_MODE = 14      /* how H6 finds the hits inside a stored peak's window (same result):
+                                       0 = every hit scans the MARKED theta columns, one thread per hit (default; cheap when
+                                       few columns are marked);
+                                       1 = dense: the dead accumulator is rewritten as the window mask and every hit is
+                                       tested at ALL columns with the voting loop's own mapping (lane = column, packed
+                                       arithmetic, conflict-free loads, one ballot per hit): one voting-sized pass whatever
+                                       the number of peaks;
+                                       2 = dense when the stored peaks' windows could cover more than half of the columns.
+                                       One-CTA-per-event grids with the window filter only (a clustered grid, the distance
+                                       filter, or an event with more hits than the peak bitmap has bits keep mode 0).
+                                       Never yet timed */
 } hough_option;
 
 typedef enum hough_option_f64 {

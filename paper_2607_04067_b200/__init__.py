@@ -30,6 +30,7 @@ HOUGH_OPT_THETA_WRAP = 10
 HOUGH_OPT_KEEP_MODE = 11
 HOUGH_OPT_STAGING = 12
 HOUGH_OPT_SCHEDULER = 13
+HOUGH_OPT_SELECT_MODE = 14
 HOUGH_OPTF_KEEP_TOL = 1
 HOUGH_OPTF_B_FIELD_TESLA = 2
 HOUGH_ACC_AUTO, HOUGH_ACC_U16, HOUGH_ACC_U32 = 0, 1, 2
@@ -354,7 +355,7 @@ class Hough:
 
     def __init__(self, n_theta, n_rho, rho_max, threshold, window, max_peaks=64, acc_dtype="u16",
                  conformal_scale=1, cluster_size=0, ctas_per_sm=0, trig_table=None, peak_mode=0, rel_permille=500,
-                 nms_radius=1, theta_wrap=False, keep_mode=0, keep_tol=0.0, b_field=1.0, staging=0, scheduler=0):
+                 nms_radius=1, theta_wrap=False, keep_mode=0, keep_tol=0.0, b_field=1.0, staging=0, scheduler=0, select_mode=0):
         self.n_theta, self.n_rho, self.max_peaks = n_theta, n_rho, max_peaks
         self.ctx = hough_create(n_theta, n_rho, float(rho_max), threshold, window)
         try:
@@ -383,6 +384,8 @@ class Hough:
                 hough_set_option(self.ctx, HOUGH_OPT_STAGING, staging)
             if scheduler:
                 hough_set_option(self.ctx, HOUGH_OPT_SCHEDULER, scheduler)
+            if select_mode:
+                hough_set_option(self.ctx, HOUGH_OPT_SELECT_MODE, select_mode)
         except Exception:
             self.close()
             raise

@@ -82,7 +82,7 @@ struct hough_ctx {
     int opt_cluster = 0;
     int opt_ctas_per_sm = 0;
     int opt_vote_path = 0;
-    int peak_mode = 0, rel_permille = 500, nms_radius = 1, theta_wrap = 0, keep_mode = 0, stage_mode = 0, sched_mode = 0;
+    int peak_mode = 0, rel_permille = 500, nms_radius = 1, theta_wrap = 0, keep_mode = 0, stage_mode = 0, sched_mode = 0, select_mode = 0;
     double keep_tol = 0.0, b_field = 1.0;
     int device = 0;
     int sm_count = 0;
@@ -121,7 +121,7 @@ const void* pick_kernel(bool acc16, bool cl, int cpl, bool ext) {
     return cl ? kernel_ptr<false, true, false>(cpl) : kernel_ptr<false, false, false>(cpl);
 }
 
-bool wants_ext(const hough_ctx* c) { return c->peak_mode != 0 || c->theta_wrap != 0 || c->keep_mode != 0 || c->stage_mode != 0 || c->sched_mode != 0; }
+bool wants_ext(const hough_ctx* c) { return c->peak_mode != 0 || c->theta_wrap != 0 || c->keep_mode != 0 || c->stage_mode != 0 || c->sched_mode != 0 || c->select_mode != 0; }
 
 // cudaFuncAttributeMaxDynamicSharedMemorySize belongs to the kernel (per device), not to a handle: several live
 // handles may share one instantiation with different footprints, so the attribute is only ever RAISED.
@@ -359,6 +359,7 @@ int launch(hough_ctx* c, const hough_io* io, cudaStream_t stream) {
     kp.theta_wrap = c->theta_wrap; kp.keep_mode = c->keep_mode; kp.keep_tol = c->keep_tol;
     kp.stage_mode = c->stage_mode;
     kp.sched_mode = c->sched_mode;
+    kp.select_mode = c->select_mode;
     if ((c->stage_mode == 1 || c->sched_mode == 1) && ((uintptr_t)io->d_xy & 15u) != 0)
         return fail(HOUGH_ERR_INVALID_ARG, "bulk-copy staging and the work-stealing scheduler need d_xy 16-byte aligned");
     if (c->sched_mode == 1 && (long long)io->n_events * pl.csize > 0x7FFFFFF0LL)
@@ -463,6 +464,9 @@ int hough_set_option(hough_ctx* c, int key, long long value) {
         case HOUGH_OPT_SCHEDULER:
             if (value != 0 && value != 1) return fail(HOUGH_ERR_INVALID_ARG, "scheduler must be 0 or 1");
             c->sched_mode = (int)value; return HOUGH_OK;
+        case HOUGH_OPT_SELECT_MODE:
+            if (value < 0 || value > 2) return fail(HOUGH_ERR_INVALID_ARG, "select mode must be 0, 1 or 2");
+            c->select_mode = (int)value; return HOUGH_OK;
         default: break;
     }
     switch (key) {

@@ -107,6 +107,7 @@ struct KParams {
     int keep_mode;        // 0: (theta, rho) window; 1: distance to the candidate circle
     int circ_cap;         // distance filter: circles staged in the dead accumulator region
     int stage_mode;       // 0: coalesced float2 loads; 1: one cp.async.bulk per chunk into the hit buffer (north_star (1))
+    int select_mode;      // H6: 0 scan of the marked columns per hit; 1 dense (window mask in the accumulator, vote mapping); 2 dense when many columns are marked
     int sched_mode;       // 0: one CTA per event; 1: a resident CTA steals not-yet-launched CTAs' events (cluster launch control)
     double keep_tol;      // distance filter tolerance, units of the hit coordinates
 };
@@ -889,7 +890,84 @@ __global__ void __launch_bounds__(1024, 1) hough_event_kernel(const __grid_const
         int* colq = (int*)(acc + p.colq_off);
         int n_marked = 0, n_g8 = 0, n_circ = 0;
         double* circ = (double*)(acc + p.w8_off);   // EXT, distance filter: (x_c, y_c, r_c) of the first circ_cap stored peaks
-        if (EXT && p.keep_mode == 1) {
+        // ---- H6 dense mode (EXT, HOUGH_OPT_SELECT_MODE).  When most theta columns are marked, the scan
+        // below costs more than the voting phase (every hit x every marked column, one thread per hit).  Here the dead
+        // accumulator is rewritten as the window mask -- cell (j, k) non-zero iff some stored peak has |j - j_p| <= w and
+        // |k - k_p| <= w, S5's union of windows -- and every hit is tested at ALL columns with the voting loop's own
+        // mapping and address arithmetic, a load where the vote had its atomic: bins outside the grid read the trash
+        // row (zero).  One ballot per hit; the keep flags (one bit per hit of the event) live in the dead peak bitmap.
+        const int ev_tame_d = (EXT && p.select_mode != 0) ? misc[33] : 0;
+        unsigned* kf = pbm;
+        bool dense = false;
+        if (EXT && !CL && p.select_mode != 0 && p.keep_mode == 0 && n_stored > 0 && n > 0 && (long long)n <= 8LL * p.pbm_bytes &&
+            (p.select_mode == 1 || 2LL * n_stored * (2 * p.window + 1) > p.n_theta)) {
+            dense = true;
+            {
+                uint4* z = (uint4*)smem;
+                const uint4 zz = make_uint4(0, 0, 0, 0);
+                for (int i = tid; i < zero_vec; i += nthreads) z[i] = zz;      // accumulator, trash row, peak bitmap (= flags)
+            }
+            __syncthreads();
+            for (int q = tid; q < n_stored; q += nthreads) {
+                const hough_peak pk = p.peaks[(size_t)e * p.max_peaks + q];
+                for (int dj = -p.window; dj <= p.window; ++dj) {
+                    int j = (int)pk.theta_bin + dj, kref = (int)pk.rho_bin;
+                    if (j < 0 || j >= p.n_theta) {
+                        if (!p.theta_wrap) continue;
+                        while (j < 0) { j += p.n_theta; kref = p.n_rho - 1 - kref; }       // reading Q19: mirrored across the seam
+                        while (j >= p.n_theta) { j -= p.n_theta; kref = p.n_rho - 1 - kref; }
+                    }
+                    const unsigned half = ACC16 ? (1u << (16 * ((j >> 5) & 1))) : 1u;
+                    for (int k = max(0, kref - p.window); k <= min(p.n_rho - 1, kref + p.window); ++k) {
+                        const unsigned woff = (unsigned)k * pitch + 4u * cell_word_off<ACC16>(j);
+                        if (HB_CHK(j < ncols && woff + 4 <= limit, HB_H6_SETUP)) atomicOr((unsigned*)(acc + woff), half);
+                    }
+                }
+            }
+            __syncthreads();
+            const int S = p.n_stripes;
+            for (int cbeg = 0; cbeg < n; cbeg += chunk) {
+                const int m = min(chunk, n - cbeg);
+                if (!single) {                    // the staged (u, v) of a chunked event are gone: stage this chunk again
+                    for (int i = tid; i < m; i += nthreads)
+                        if (HB_CHK(i < p.chunk, HB_STAGE)) hb0[i] = conformal(__ldg(&p.xy[beg + cbeg + i]), p.scale);
+                    __syncthreads();
+                }
+                const float2* src = single ? hb : hb0;
+                for (int i = stripe; i < m; i += S) {
+                    const float2 uv = src[i];
+                    unsigned any = 0;
+                    if (ev_tame_d) {
+#pragma unroll
+                        for (int q = 0; q < CPL; q += 2) {
+                            unsigned b0, b1;
+                            bin_bits2(uv.x, uv.y, c2q[q / 2], s2q[q / 2], rho_max, inv, b0, b1);
+                            const unsigned rel0 = min(b0 * pitch + lc0, trash0) + (ACC16 ? 128 * (q / 2) : 128 * q);
+                            const unsigned rel1 = min(b1 * pitch + lc0, trash0) + (ACC16 ? 128 * (q / 2) : 128 * (q + 1));
+                            const unsigned w0 = HB_CHK(rel0 + 4 <= acc_end, HB_KEEP) ? *(const unsigned*)(acc + rel0) : 0u;
+                            const unsigned w1 = HB_CHK(rel1 + 4 <= acc_end, HB_KEEP) ? *(const unsigned*)(acc + rel1) : 0u;
+                            any |= ACC16 ? ((w0 & 0xFFFFu) | (w1 >> 16)) : (w0 | w1);
+                        }
+                    } else {                      // degenerate hits somewhere in the event: the literal S2, as on the slow vote path
+                        for (int q = 0; q < CPL; ++q) {
+                            const int jl = 32 * (g * CPL + q) + lane;
+                            if (jl >= ncols) continue;
+                            const int k = bin_exact(uv.x, uv.y, p.cos_t[col0 + jl], p.sin_t[col0 + jl], p.rho_max, p.inv, p.n_rho);
+                            if (k < 0) continue;
+                            const unsigned woff = (unsigned)k * pitch + 4u * cell_word_off<ACC16>(jl);
+                            const unsigned wv = HB_CHK(woff + 4 <= limit, HB_KEEP) ? *(const unsigned*)(acc + woff) : 0u;
+                            any |= ACC16 ? ((wv >> (16 * ((jl >> 5) & 1))) & 0xFFFFu) : wv;
+                        }
+                    }
+                    const unsigned bal = __ballot_sync(0xffffffffu, any != 0u);
+                    if (lane == 0 && bal && HB_CHK(4 * ((cbeg + i) >> 5) + 4 <= p.pbm_bytes, HB_KEEP))
+                        atomicOr(&kf[(cbeg + i) >> 5], 1u << ((cbeg + i) & 31));       // the column groups of one hit are different warps
+                }
+                __syncthreads();                  // flags complete / hb0 free for the next chunk
+            }
+        }
+        if (dense) {
+        } else if (EXT && p.keep_mode == 1) {
             // ---- N4b set-up (reading Q20): the stored peaks' candidate circles, Eq. (2)
             n_circ = min(n_stored, p.circ_cap);
             for (int q = tid; q < n_circ; q += nthreads) {
@@ -1049,7 +1127,7 @@ __global__ void __launch_bounds__(1024, 1) hough_event_kernel(const __grid_const
                 if (valid) uv = single ? hb[i] : conformal(__ldg(&p.xy[beg + i]), p.scale);
                 float2 hxy = make_float2(0.0f, 0.0f);
                 if (EXT && p.keep_mode == 1 && valid) hxy = __ldg(&p.xy[beg + i]);
-                const bool kp = keep_test(uv, hxy, valid);
+                const bool kp = (EXT && dense) ? (valid && ((kf[i >> 5] >> (i & 31)) & 1u) != 0u) : keep_test(uv, hxy, valid);
                 int blk_total;
                 const int ppos = block_exscan(kp ? 1 : 0, misc, blk_total);
                 if (valid) {

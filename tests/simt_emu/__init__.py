@@ -113,7 +113,7 @@ def _race_reports(exe: str, stderr: str):
 def run(xy, off, n_theta, n_rho, rho_max, threshold, window, table, max_peaks=64, acc_dtype="u16", accum=True,
         conformal_scale=1, cluster_size=0, ctas_per_sm=0, vote_path=0, grid_clusters=0, debug_bounds=False, timeout=900,
         peak_mode=0, rel_permille=500, nms_radius=1, theta_wrap=False, keep_mode=0, keep_tol=0.0, b_field=1.0, circles=False,
-        order=None, staging=0, scheduler=0, steals=None, race=False, exe=None):
+        order=None, staging=0, scheduler=0, steals=None, race=False, exe=None, select_mode=0):
     """Same arguments and result keys as tests/test_parity_gpu.py::gpu_run."""
     import paper_2607_04067_b200 as hb
     xy = np.ascontiguousarray(xy, dtype=np.float32).reshape(-1, 2)
@@ -131,7 +131,7 @@ def run(xy, off, n_theta, n_rho, rho_max, threshold, window, table, max_peaks=64
     head = [n_theta, n_rho, threshold, window, max_peaks, int(plan["acc_bits"] == 16), int(plan["cluster_size"] > 1),
             plan["cols_per_lane"], plan["cluster_size"], plan["threads"], plan["smem_bytes"], int(vote_path == 1),
             n_events, n_total, 1, int(accum), grid_clusters, peak_mode, rel_permille, nms_radius, int(bool(theta_wrap)), keep_mode,
-            int(circles), int(staging) | (int(scheduler) << 1)]
+            int(circles), int(staging) | (int(scheduler) << 1) | (int(select_mode) << 2)]
     with tempfile.TemporaryDirectory() as d:
         fin, fout = os.path.join(d, "in.bin"), os.path.join(d, "out.bin")
         with open(fin, "wb") as f:

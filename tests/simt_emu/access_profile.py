@@ -4,7 +4,9 @@ access of tracked memory per code address).  Not a timing and not a hardware cou
 phase does on a given workload, e.g. how many (hit, marked column) evaluations H6 makes against the (hit, column)
 votes of H3.  Phases are the `// ----` section comments of hough_kernel.cuh.
 
-    python tests/simt_emu/access_profile.py [config events]...      (default: 1 8  2 4  3 3)
+    python tests/simt_emu/access_profile.py [--select MODE] [config events]...      (default: 1 8  2 4  3 3)
+
+--select: HOUGH_OPT_SELECT_MODE of the run (0 scan, 1 dense, 2 auto).
 """
 import os
 import re
@@ -16,6 +18,9 @@ sys.path.insert(0, os.path.dirname(os.path.dirname(HERE)))
 
 
 def main(argv):
+    select = 0
+    if argv[:1] == ["--select"]:
+        select, argv = int(argv[1]), argv[2:]
     os.environ["HOUGH_EMU_PROFILE"] = "1"
     import simt_emu
     import stcf_inputs as si
@@ -33,15 +38,15 @@ def main(argv):
         w = si.config(cfg)
         xy, off, _ = si.generate(w, nev)
         r = simt_emu.run(xy, off, w.n_theta, w.n_rho, w.rho_max, w.threshold, w.window, si.trig_table(w.n_theta), max_peaks=w.max_peaks,
-                         acc_dtype=w.acc_dtype, accum=False, race=True)
+                         acc_dtype=w.acc_dtype, accum=False, race=True, select_mode=select)
         agg = {}
         for (loc, space, kind), n in r["profile"].items():
             m = re.search(r":(\d+)", loc)
             key = (phase(int(m.group(1))) if m else loc, space, kind)
             agg[key] = agg.get(key, 0) + n
         n_hits = len(xy)
-        print("\n%s: %d events, %d hits, %d x %d %s, %d threads; stored peaks per event %.0f, kept fraction %.2f"
-              % (w.name, nev, n_hits, w.n_theta, w.n_rho, w.acc_dtype, r["info"]["THREADS"], r["counts"][:, 0].clip(max=w.max_peaks).mean(),
+        print("\n%s%s: %d events, %d hits, %d x %d %s, %d threads; stored peaks per event %.0f, kept fraction %.2f"
+              % (w.name, " (select mode %d)" % select if select else "", nev, n_hits, w.n_theta, w.n_rho, w.acc_dtype, r["info"]["THREADS"], r["counts"][:, 0].clip(max=w.max_peaks).mean(),
                  r["counts"][:, 1].sum() / max(1, n_hits)))
         print("| phase | memory | access | thread-level operations | per hit |\n|---|---|---|---|---|")
         for k, n in sorted(agg.items(), key=lambda kv: -kv[1]):

@@ -60,8 +60,8 @@ int main(int argc, char** argv) {
     g_acc16 = h[5]; g_cl = h[6]; g_cpl = h[7];
     const int csize = h[8], threads = h[9], smem_bytes = h[10], force_slow = h[11], n_events = h[12], n_total = h[13];
     const int want_kept = h[14], want_accum = h[15], grid_clusters = h[16];
-    const int peak_mode = h[17], rel_permille = h[18], nms_radius = h[19], theta_wrap = h[20], keep_mode = h[21], want_circles = h[22], stage_mode = h[23] & 1, sched_mode = (h[23] >> 1) & 1;
-    g_ext = peak_mode != 0 || theta_wrap != 0 || keep_mode != 0 || stage_mode != 0 || sched_mode != 0;
+    const int peak_mode = h[17], rel_permille = h[18], nms_radius = h[19], theta_wrap = h[20], keep_mode = h[21], want_circles = h[22], stage_mode = h[23] & 1, sched_mode = (h[23] >> 1) & 1, select_mode = (h[23] >> 2) & 3;
+    g_ext = peak_mode != 0 || theta_wrap != 0 || keep_mode != 0 || stage_mode != 0 || sched_mode != 0 || select_mode != 0;
     std::vector<float> cos_t(n_theta), sin_t(n_theta);
     rd(f, cos_t.data(), n_theta); rd(f, sin_t.data(), n_theta);
     emu::Guarded b_off, b_xy, b_keep, b_peaks, b_counts, b_kxy, b_kidx, b_acc;
@@ -115,7 +115,7 @@ int main(int argc, char** argv) {
     kp.colq_off = plan[20]; kp.stash_off = plan[21]; kp.cnt_off = plan[22]; kp.gcnt_off = plan[23];
     kp.rcp_groups = (unsigned)plan[24]; kp.rcp_2s = (unsigned)plan[25]; kp.circ_cap = plan[26];
     kp.peak_mode = peak_mode; kp.rel_permille = rel_permille; kp.nms_radius = nms_radius; kp.theta_wrap = theta_wrap;
-    kp.keep_mode = keep_mode; kp.keep_tol = dbl[0]; kp.stage_mode = stage_mode; kp.sched_mode = sched_mode;
+    kp.keep_mode = keep_mode; kp.keep_tol = dbl[0]; kp.stage_mode = stage_mode; kp.sched_mode = sched_mode; kp.select_mode = select_mode;
     kp.vpr = kp.pitch_b / 16;
     if (plan[0] != csize || plan[1] != threads || plan[2] != smem_bytes || plan[4] != g_cpl || (plan[3] == 16) != (g_acc16 != 0))
         emu::die("header and plan disagree");

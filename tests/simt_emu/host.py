@@ -101,7 +101,7 @@ class Handle:
 
     def __init__(self, n_theta, n_rho, rho_max, threshold, window, table, max_peaks=64, acc_dtype="u16", conformal_scale=1,
                  cluster_size=0, ctas_per_sm=0, vote_path=0, peak_mode=0, rel_permille=None, nms_radius=None, theta_wrap=False,
-                 keep_mode=0, keep_tol=None, b_field=None, staging=0, scheduler=0, race=False):
+                 keep_mode=0, keep_tol=None, b_field=None, staging=0, scheduler=0, select_mode=0, race=False):
         import paper_2607_04067_b200 as hb
         self.hb, self.lib = hb, load(race)
         self.n_theta, self.n_rho, self.max_peaks = n_theta, n_rho, max_peaks
@@ -113,7 +113,7 @@ class Handle:
                        (hb.HOUGH_OPT_CLUSTER_SIZE, cluster_size), (hb.HOUGH_OPT_CTAS_PER_SM, ctas_per_sm), (hb.HOUGH_OPT_VOTE_PATH, vote_path),
                        (hb.HOUGH_OPT_PEAK_MODE, peak_mode), (hb.HOUGH_OPT_REL_THRESHOLD_PERMILLE, rel_permille), (hb.HOUGH_OPT_NMS_RADIUS, nms_radius),
                        (hb.HOUGH_OPT_THETA_WRAP, int(bool(theta_wrap))), (hb.HOUGH_OPT_KEEP_MODE, keep_mode), (hb.HOUGH_OPT_STAGING, staging),
-                       (hb.HOUGH_OPT_SCHEDULER, scheduler)):
+                       (hb.HOUGH_OPT_SCHEDULER, scheduler), (hb.HOUGH_OPT_SELECT_MODE, select_mode)):
             if v is not None and v != 0 or key in (hb.HOUGH_OPT_MAX_PEAKS, hb.HOUGH_OPT_ACC_DTYPE):
                 self.check(self.lib.hough_set_option(self.ctx, key, int(v)), "hough_set_option(%d)" % key)
         for key, v in ((hb.HOUGH_OPTF_KEEP_TOL, keep_tol), (hb.HOUGH_OPTF_B_FIELD_TESLA, b_field)):

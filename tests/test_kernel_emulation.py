@@ -83,7 +83,7 @@ def emu_ex(w, xy, off, accum=True, circles=False, **kw):
     base = dict(max_peaks=w.max_peaks, acc_dtype=w.acc_dtype, threshold=w.threshold, window=w.window, conformal_scale=1)
     base.update({k: kw.pop(k) for k in list(kw) if k in base})
     opts = {k: kw.pop(k) for k in list(kw) if k in ("peak_mode", "rel_permille", "nms_radius", "theta_wrap", "keep_mode", "keep_tol", "b_field")}
-    emu_only = {k: kw.pop(k) for k in list(kw) if k in ("staging", "order", "scheduler", "steals")}
+    emu_only = {k: kw.pop(k) for k in list(kw) if k in ("staging", "order", "scheduler", "steals", "select_mode")}
     rho_max = kw.pop("rho_max", w.rho_max)
     g = simt_emu.run(xy, off, w.n_theta, w.n_rho, rho_max, base["threshold"], base["window"], table, max_peaks=base["max_peaks"],
                      acc_dtype=base["acc_dtype"], accum=accum, conformal_scale=base["conformal_scale"], circles=circles, **opts, **emu_only, **kw)
@@ -221,3 +221,35 @@ def test_work_stealing_scheduler_under_the_emulator(steals):
     emu_ex(w3, big, np.array([0, 7, len(big) - 3, len(big)], dtype=np.int32), scheduler=1, steals=steals, threshold=45)
     # clustered grids ignore the option
     emu_ex(w, xy, off, scheduler=1, steals=steals, cluster_size=2)
+
+
+# ---------------------------------------------------------------- H6 variant: dense selection (HOUGH_OPT_SELECT_MODE)
+@pytest.mark.parametrize("cfg,n_ev,kw", [
+    (0, 3, dict(select_mode=1, debug_bounds=True)),
+    (1, 3, dict(select_mode=1, order="shuffle:4")),
+    (2, 2, dict(select_mode=1, debug_bounds=True)),                  # 360 columns: two column groups per hit
+    (3, 2, dict(select_mode=2)),                                     # u32, ~800 peaks: the auto mode goes dense
+    (1, 3, dict(select_mode=2)),                                     # few peaks: the auto mode keeps the scan
+    (0, 3, dict(select_mode=1, theta_wrap=True)),
+    (1, 2, dict(select_mode=1, max_peaks=0)),                        # nothing stored: nothing kept, no dense pass
+    (1, 2, dict(select_mode=1, peak_mode=1, staging=1, scheduler=1, window=2)),
+    (1, 2, dict(select_mode=1, cluster_size=2)),                     # a clustered grid ignores the option
+])
+def test_dense_selection_under_the_emulator(cfg, n_ev, kw):
+    w = si.config(cfg)
+    xy, off, _ = si.generate(w, n_ev)
+    emu_ex(w, xy, off, accum=False, **kw)
+
+
+def test_dense_selection_with_degenerate_hits_and_a_chunked_event_under_the_emulator():
+    w = si.config(0)
+    xy, off, _ = si.generate(w, 3)
+    bad = np.array([[0, 0], [np.inf, 1], [1e-3, 0], [1e-20, 1e-20], [np.nan, 5], [1e30, 1e30], [3e38, 0]], dtype=np.float32)
+    xy2 = np.concatenate([xy[:off[1]], bad, xy[off[1]:]])
+    off2 = np.concatenate([[0, 0], off[1:2] + len(bad), off[2:] + len(bad), [off[-1] + len(bad)]]).astype(np.int32)
+    emu_ex(w, xy2, off2, accum=False, threshold=5, select_mode=1, grid_clusters=2, debug_bounds=True)   # the exact path of the dense test
+    w3 = si.config(3)
+    xy3, off3, _ = si.generate(w3, 3)
+    big = np.ascontiguousarray(xy3[:off3[3]])                         # one event of ~8000 hits: more than the staging chunk
+    g, _ = emu_ex(w3, big, np.array([0, len(big)], dtype=np.int32), accum=False, threshold=40, select_mode=1)
+    assert len(big) > g["info"]["CHUNK_HITS"]

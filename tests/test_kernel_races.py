@@ -58,6 +58,8 @@ SCENARIOS = {
     "N4a wrap + N4b distance filter + N1 circles, cluster of 2, bulk staging": dict(
         cfg=1, nev=3, grid_clusters=1, cluster_size=2, peak_mode=1, theta_wrap=True, keep_mode=1, keep_tol=5.0, staging=1, circles=True),
     "bulk staging + work stealing": dict(cfg=1, nev=5, grid_clusters=2, staging=1, scheduler=1),
+    "dense selection, 3 events through one CTA": dict(cfg=3, nev=3, grid_clusters=1, select_mode=1),
+    "dense selection, two column groups, shuffled": dict(cfg=2, nev=2, grid_clusters=1, select_mode=1, order="shuffle:9"),
     "work stealing, cluster of 2": dict(cfg=0, nev=3, cluster_size=2, scheduler=1),
 }
 

@@ -11,7 +11,7 @@ from tests.test_parity_gpu import compare
 pytestmark = pytest.mark.gpu
 
 OPTS = ("peak_mode", "rel_permille", "nms_radius", "theta_wrap", "keep_mode", "keep_tol", "b_field")
-GPU_ONLY = ("staging", "scheduler")          # same results by definition: the oracle has no such options
+GPU_ONLY = ("staging", "scheduler", "select_mode")          # same results by definition: the oracle has no such options
 
 
 @pytest.fixture(scope="module")
@@ -296,3 +296,27 @@ def test_work_stealing_scheduler_with_empty_refused_and_chunked_events_and_on_st
     for out in outs:
         assert np.array_equal(out["counts"].cpu().numpy(), o.counts) and np.array_equal(out["keep"].cpu().numpy(), o.keep)
     h.close()
+
+
+# ---------------------------------------------------------------- H6 variant: dense selection (the accumulator rewritten as the
+# window mask, every hit tested at all columns with the voting loop's mapping).  Same results by definition.
+@pytest.mark.parametrize("cfg,n_ev,mode,extra", [(0, 16, 1, {}), (1, 120, 1, {}), (2, 60, 1, {}), (3, 40, 1, {}), (2, 40, 2, {}), (1, 60, 2, {}),
+                                                 (5, 12, 1, {}), (0, 16, 1, dict(theta_wrap=True)), (3, 40, 1, dict(peak_mode=1, rel_permille=300, window=1)),
+                                                 (1, 50, 1, dict(staging=1, scheduler=1))])
+def test_h6_dense_selection(hb, cfg, n_ev, mode, extra):
+    w = si.config(cfg)
+    xy, off, _ = si.generate(w, n_ev)
+    gpu_ex(hb, w, xy, off, select_mode=mode, accum=False, **extra)
+
+
+def test_h6_dense_selection_with_degenerate_hits_chunked_events_and_more_hits_than_flag_bits(hb):
+    w = si.config(0)
+    xy, off, _ = si.generate(w, 3)
+    bad = np.array([[0, 0], [np.inf, 1], [1e-3, 0], [1e-20, 1e-20], [np.nan, 5], [1e30, 1e30], [3e38, 0]], dtype=np.float32)
+    xy2 = np.concatenate([xy[:off[1]], bad, xy[off[1]:]])
+    off2 = np.concatenate([[0, 0], off[1:2] + len(bad), off[2:] + len(bad), [off[-1] + len(bad)]]).astype(np.int32)
+    gpu_ex(hb, w, xy2, off2, select_mode=1, threshold=5, accum=False)
+    w3 = si.config(3)
+    xy3, off3, _ = si.generate(w3, 12)
+    cut = int(off3[6])                                                # ~17000 hits in one event: chunked, and more hits than the bitmap has bits
+    gpu_ex(hb, w3, xy3[:off3[12]], np.concatenate([[0, cut], off3[7:13]]).astype(np.int32), select_mode=1, threshold=60, accum=False)

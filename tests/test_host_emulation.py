@@ -195,6 +195,13 @@ def test_circles_and_every_option_through_the_abi():
                     cluster_size=2, staging=1, b_field=1.0, **opts)
     xy, off, _ = si.generate(w, 2)
     g = h.run(xy, off)
+    # the variants that change nothing: dense selection + work stealing on a one-CTA-per-event grid, through set_option
+    hv = host.Handle(w.n_theta, w.n_rho, w.rho_max, w.threshold, w.window, table, max_peaks=w.max_peaks, acc_dtype=w.acc_dtype,
+                     select_mode=1, scheduler=1, staging=1)
+    gv, gd = hv.run(xy, off), host.Handle(w.n_theta, w.n_rho, w.rho_max, w.threshold, w.window, table, max_peaks=w.max_peaks).run(xy, off)
+    assert all(np.array_equal(gv[k], gd[k]) for k in ("keep", "counts", "peaks", "kept_idx"))
+    assert hv.lib.hough_set_option(hv.ctx, hb.HOUGH_OPT_SELECT_MODE, 3) != hb.HOUGH_OK
+    hv.close()
     circ = h.circles(xy, off, g)
     o, oc = oracle.run_ex(xy, off, w.n_theta, w.n_rho, w.rho_max, w.threshold, w.window, table[0], table[1], max_peaks=w.max_peaks,
                           acc_u16=True, want_circles=True, n_threads=4, **opts)

@@ -300,9 +300,9 @@ def test_work_stealing_scheduler_with_empty_refused_and_chunked_events_and_on_st
 
 # ---------------------------------------------------------------- H6 variant: dense selection (the accumulator rewritten as the
 # window mask, every hit tested at all columns with the voting loop's mapping).  Same results by definition.
-@pytest.mark.parametrize("cfg,n_ev,mode,extra", [(0, 16, 1, {}), (1, 120, 1, {}), (2, 60, 1, {}), (3, 40, 1, {}), (2, 40, 2, {}), (1, 60, 2, {}),
-                                                 (5, 12, 1, {}), (0, 16, 1, dict(theta_wrap=True)), (3, 40, 1, dict(peak_mode=1, rel_permille=300, window=1)),
-                                                 (1, 50, 1, dict(staging=1, scheduler=1))])
+@pytest.mark.parametrize("cfg,n_ev,mode,extra", [(0, 16, 1, {}), (1, 40, 1, {}), (2, 24, 1, {}), (3, 12, 1, {}), (2, 12, 2, {}), (1, 30, 2, {}),
+                                                 (5, 8, 1, {}), (0, 16, 1, dict(theta_wrap=True)), (3, 8, 1, dict(peak_mode=1, rel_permille=300, window=1)),
+                                                 (1, 20, 1, dict(staging=1, scheduler=1))])
 def test_h6_dense_selection(hb, cfg, n_ev, mode, extra):
     w = si.config(cfg)
     xy, off, _ = si.generate(w, n_ev)

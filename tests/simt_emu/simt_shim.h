@@ -92,6 +92,7 @@ struct Barrier {
     unsigned gen = 0;
     int acc_and = 1, acc_or = 0, acc_cnt = 0;
     int res_and = 1, res_or = 0, res_cnt = 0;
+    int line = 0;                    // synccheck: the source line of the barrier call the first thread of this generation made
 };
 
 struct Warp {
@@ -289,8 +290,17 @@ EMU_NOSAN inline void yield() {
     swapcontext(&me->ctx, &g.sched);
 }
 
-EMU_NOSAN inline void wait_barrier(Barrier& b, int pred, int& r_and, int& r_or, int& r_cnt, int scope = 1) {
+// synccheck: every thread of a barrier generation must arrive from the SAME barrier call of the source (a barrier in
+// divergent code pairs up calls that were never meant to meet; the hardware would count them all the same).  `line` is
+// the call site (__builtin_LINE() in the default arguments of __syncthreads* / cluster.sync).
+EMU_NOSAN inline void wait_barrier(Barrier& b, int pred, int& r_and, int& r_or, int& r_cnt, int scope = 1, int line = 0) {
     const unsigned gen = b.gen;
+    if (b.arrived == 0) b.line = line;
+    else if (b.line != line) {
+        fprintf(stderr, "simt_emu: threads of one %s barrier generation arrive from different source lines: %d and %d\n",
+                scope == 2 ? "cluster" : "CTA", b.line, line);
+        die("divergent barrier");
+    }
     b.acc_and &= pred ? 1 : 0;
     b.acc_or |= pred ? 1 : 0;
     b.acc_cnt += pred ? 1 : 0;
@@ -518,10 +528,10 @@ inline dim3& blockDim = emu::g.bdim;      // (objects, not macros: host code has
 inline dim3& gridDim = emu::g.gdim;
 #define HOUGH_DYN_SMEM(name) unsigned char* name = emu::dyn_smem()
 
-EMU_NOSAN inline void __syncthreads() { int a, o, c; emu::wait_barrier(emu::cur->cta->bar, 1, a, o, c); }
-EMU_NOSAN inline int __syncthreads_and(int p) { int a, o, c; emu::wait_barrier(emu::cur->cta->bar, p, a, o, c); return a; }
-EMU_NOSAN inline int __syncthreads_or(int p) { int a, o, c; emu::wait_barrier(emu::cur->cta->bar, p, a, o, c); return o; }
-EMU_NOSAN inline int __syncthreads_count(int p) { int a, o, c; emu::wait_barrier(emu::cur->cta->bar, p, a, o, c); return c; }
+EMU_NOSAN inline void __syncthreads(int line = __builtin_LINE()) { int a, o, c; emu::wait_barrier(emu::cur->cta->bar, 1, a, o, c, 1, line); }
+EMU_NOSAN inline int __syncthreads_and(int p, int line = __builtin_LINE()) { int a, o, c; emu::wait_barrier(emu::cur->cta->bar, p, a, o, c, 1, line); return a; }
+EMU_NOSAN inline int __syncthreads_or(int p, int line = __builtin_LINE()) { int a, o, c; emu::wait_barrier(emu::cur->cta->bar, p, a, o, c, 1, line); return o; }
+EMU_NOSAN inline int __syncthreads_count(int p, int line = __builtin_LINE()) { int a, o, c; emu::wait_barrier(emu::cur->cta->bar, p, a, o, c, 1, line); return c; }
 inline void __threadfence() {}
 
 EMU_NOSAN inline void need_full_mask(unsigned m) { if (m != 0xffffffffu) emu::die("only full-mask warp collectives are emulated"); }
@@ -599,7 +609,7 @@ inline unsigned min(unsigned a, int b) { return a < (unsigned)b ? a : (unsigned)
 namespace cooperative_groups {
 struct cluster_group {
     EMU_NOSAN unsigned block_rank() const { return (unsigned)emu::cur->cta->rank; }
-    EMU_NOSAN void sync() const { int a, o, c; emu::wait_barrier(emu::g.cluster_bar, 1, a, o, c, 2); }
+    EMU_NOSAN void sync(int line = __builtin_LINE()) const { int a, o, c; emu::wait_barrier(emu::g.cluster_bar, 1, a, o, c, 2, line); }
     EMU_NOSAN void* map_shared_rank(void* p, int rank) const {
         const ptrdiff_t off = (unsigned char*)p - emu::cur->cta->smem.ptr;
         if (off < 0 || (size_t)off >= emu::cur->cta->smem.bytes) emu::die("map_shared_rank of a pointer outside shared memory");

@@ -131,3 +131,19 @@ def test_mutant_is_reported(mutant_exes, name):
         for m in re.finditer(r"emu_mut\d+\.cuh:(\d+)", r["now"] + " " + r["earlier"]):
             lines.append(src[int(m.group(1)) - 1])
     assert any(needle in l for l in lines), (needle, lines[:6], str(info.value)[:1500])
+
+
+def test_synccheck_a_barrier_reached_from_two_call_sites_is_refused():
+    """The emulator's synccheck: all threads of a barrier generation must come from the same barrier call of the source."""
+    d = tempfile.mkdtemp(prefix="hough_mut_")
+    try:
+        exe = simt_emu.build_mutant(os.path.join(d, "emu_sync"), [
+            ("            __syncthreads();   // D / lists are dead: the region may be zeroed for the next event",
+             "            if (tid & 32) __syncthreads();\n            else __syncthreads();")], race=False)
+        w = si.config(0)
+        xy, off, _ = si.generate(w, 1)
+        with pytest.raises(RuntimeError, match="divergent barrier"):
+            simt_emu.run(xy, off, w.n_theta, w.n_rho, w.rho_max, w.threshold, w.window, si.trig_table(w.n_theta), max_peaks=w.max_peaks,
+                         acc_dtype=w.acc_dtype, accum=False, exe=exe)
+    finally:
+        shutil.rmtree(d, ignore_errors=True)
